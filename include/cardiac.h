@@ -1,0 +1,166 @@
+/*
+ * cardiac.h — C ABI of libcardiac.so: the fully explicit FP64 time step of the 2-D
+ * reaction-diffusion system  dz/dt = D lap(z) + N[z]  (Eq. 1) with no-flux
+ * boundaries (Eq. 2) for the FitzHugh-Nagumo (Eq. 3),
+ * Karma (Eq. 4) and Bueno-Orovio-Cherry-Fenton (Eq. 5)
+ * models, on one NVIDIA B200 (sm_100a).
+ *
+ * Everything behind this boundary is CUDA; there is no CPU fallback.  Every function that
+ * touches the device fails with CARDIAC_ERR_CUDA when no usable device is present.
+ *
+ * Conventions
+ *   - "state" is a dense float64 array [batch][n_v][ny][nx], x fastest (row-adjacent
+ *     cells adjacent in memory).  Field order: FHN (u,v); Karma (u,v); BOCF (u,v,w,s).
+ *   - Pointers are tagged host/device by an explicit int flag; device pointers must be valid
+ *     on the CUDA device that was current when the context was created.
+ *   - The caller owns every buffer it passes in (state arrays, the stream, a bound workspace)
+ *     and must keep the stream and workspace alive until cardiac_destroy.  The library owns the
+ *     context and anything it allocated itself.
+ *   - cardiac_step and device-side set/get are enqueued on the context stream and return
+ *     without synchronising; host-side set/get synchronise that stream before returning.
+ *   - All functions returning int return CARDIAC_OK (0) or a negative error code;
+ *     cardiac_last_error gives the text.  The library never checks stability (dt against
+ *     dx^2/4D) nor NaN/Inf in the state.
+ *   - step(a); step(b) is bitwise identical to step(a+b) as long as the same execution plan is
+ *     used (cardiac_set_plan), results do not depend on the batch position of a member, and
+ *     repeated runs are bitwise identical (no atomics on data, fixed summation order).
+ */
+#ifndef CARDIAC_H
+#define CARDIAC_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cardiac_ctx cardiac_ctx; /* opaque, owned by the library */
+
+/* model ("three different models") */
+enum { CARDIAC_FHN = 0, CARDIAC_KARMA = 1, CARDIAC_BOCF = 2 };
+
+/* scheme = stencil | integrator | boundary | variant */
+enum {
+  /* bits 0-7: Laplacian stencil (Eq. 6).  dx = dy.      */
+  CARDIAC_LAP5   = 0, /* Eq. 6 with alpha_a = 1, alpha_d = 0: (sum of 4 axial nbrs - 4 U)/dx^2 */
+  CARDIAC_LAP9X4 = 1, /* radius-2 cross, per axis (-1,16,-30,16,-1)/(12 dx^2): the "larger stencil"
+                         of PAPER.md:114, 4th order                                            */
+  CARDIAC_BOX9   = 2, /* Eq. 6 with alpha_a = 2/3, alpha_d = 1/6, centre -10/3 (isotropic 3x3) */
+  /* bits 8-15: time integrator.  Fixed dt.                                  */
+  CARDIAC_EULER  = 0 << 8, /* z+ = z + dt f(z)                                                  */
+  CARDIAC_HEUN   = 1 << 8, /* Y2 = z + dt f(z); z+ = z + dt/2 (f(z) + f(Y2))                    */
+  CARDIAC_RK4    = 2 << 8, /* classic Runge-Kutta                                               */
+  CARDIAC_RUSH_LARSEN   = 3 << 8, /* BOCF only: u by explicit Euler, gates x' = a x + b by the
+                                     exponential update                      */
+  CARDIAC_IMPLICIT_EULER = 4 << 8, /* BOCF only: u explicit, gates by pointwise implicit Euler  */
+  /* bits 16-23: boundary condition                                                             */
+  CARDIAC_NOFLUX   = 0 << 16, /* mirror about the boundary node: U[-m] = U[m], U[N-1+m] = U[N-1-m],
+                                 each axis independently (PAPER.md:104 Fig. 1, :114)            */
+  CARDIAC_PERIODIC = 1 << 16, /* "mapping to the opposite-edge values"           */
+  /* bits 24-31: model variant                                                                  */
+  CARDIAC_VARIANT_PAPER    = 0 << 24, /* equations as printed                                   */
+  CARDIAC_VARIANT_TANHFREE = 1 << 24  /* tanh(x) -> 2 H_k'(x) - 1 (k' = param)     */
+};
+
+/* execution plan (how the same numbers are produced) */
+enum {
+  CARDIAC_PLAN_AUTO       = 0, /* library picks by (model, scheme, nx*ny*batch)                 */
+  CARDIAC_PLAN_STAGE      = 1, /* one fused stencil+reaction+RK-stage launch per substep        */
+  CARDIAC_PLAN_FUSED      = 2, /* all substeps of one time step (or several Euler steps) on chip,
+                                  overlapped tiles, one launch                                  */
+  CARDIAC_PLAN_PERSISTENT = 3  /* one cooperative launch for all nsteps; tiles resident on chip,
+                                  neighbour halo exchange through L2                            */
+};
+
+/* error codes */
+enum {
+  CARDIAC_OK = 0,
+  CARDIAC_ERR_INVALID   = -1, /* invalid argument                                               */
+  CARDIAC_ERR_CUDA      = -2, /* CUDA runtime error (text in cardiac_last_error)                */
+  CARDIAC_ERR_NOSTATE   = -3, /* step/get_state before set_state                                */
+  CARDIAC_ERR_WORKSPACE = -4  /* bound workspace too small or misaligned                        */
+};
+
+/* Number of fields n_v of a model: 2, 2, 4; -1 for an unknown model. */
+int cardiac_num_fields(int model);
+
+/* Number of entries of the model's parameter block (5, 9, 30); -1 for an unknown model.
+ *   FHN  : D_u, delta(=D_v), epsilon, a1, a0
+ *   Karma: gamma, tau_u, tau_v, u_h, u_v, u_star, Re, M, k
+ *   BOCF : D, k, u_o, u_u, theta_v, theta_w, theta_v_minus, theta_o, tau_v1_minus, tau_v2_minus,
+ *          tau_v_plus, tau_w1_minus, tau_w2_minus, k_w_minus, u_w_minus, tau_w_plus, tau_fi,
+ *          tau_o1, tau_o2, tau_so1, tau_so2, k_so, u_so, tau_s1, tau_s2, k_s, u_s, tau_si,
+ *          tau_w_inf, w_inf_star                                    (Q9) */
+int cardiac_num_params(int model);
+
+/* Copy the library's default parameter block of `model` into p[0..n-1] (host). n must equal
+ * cardiac_num_params(model). */
+int cardiac_default_params(int model, double* p, int n);
+
+/* Create a context for `batch` independent states of nx*ny cells (N x N grid, spacing
+ * dx = dy, fixed dt; nx != ny allowed).  Requires nx, ny >= 2r+1 (r = stencil radius), batch >= 1,
+ * finite dx > 0 and dt > 0, known model/scheme bits, Rush-Larsen / implicit Euler only with BOCF.
+ * The current CUDA device is captured.  Returns NULL on failure (text: cardiac_last_error(NULL)). */
+cardiac_ctx* cardiac_create(int model, int nx, int ny, double dx, double dt, int scheme, int batch);
+
+/* Replace the model parameters (host array, n == cardiac_num_params(model)).  Takes effect for
+ * subsequent steps.  M (Karma) must be an integer in [1, 16]. */
+int cardiac_set_params(cardiac_ctx*, const double* p, int n);
+
+/* Read back the active parameter block (host array). */
+int cardiac_get_params(const cardiac_ctx*, double* p, int n);
+
+/* Use `cuda_stream` (a cudaStream_t passed as void*, e.g. torch.cuda.current_stream().cuda_stream;
+ * NULL = legacy default stream) for all subsequent work. */
+int cardiac_set_stream(cardiac_ctx*, void* cuda_stream);
+
+/* Choose the execution plan (CARDIAC_PLAN_*).  CARDIAC_ERR_INVALID if the plan does not support
+ * the context's (model, scheme, size). `param` is plan specific: FUSED + Euler = time steps per
+ * launch (0 = default); otherwise 0. */
+int cardiac_set_plan(cardiac_ctx*, int plan, int param);
+
+/* The plan that cardiac_step will use (resolved from AUTO). */
+int cardiac_get_plan(const cardiac_ctx*);
+
+/* Bytes of device workspace the context needs (all stage buffers and halos). */
+size_t cardiac_workspace_bytes(const cardiac_ctx*);
+
+/* Bind caller-allocated device memory (256-byte aligned, >= cardiac_workspace_bytes) as the
+ * workspace; must be called before the first set_state, else the library cudaMallocs its own. */
+int cardiac_bind_workspace(cardiac_ctx*, void* dev_ptr, size_t bytes);
+
+/* Copy a dense [batch][n_v][ny][nx] float64 state into the context. src_on_device != 0: src is a
+ * device pointer, the copy is enqueued on the stream.  Otherwise src is a host pointer and the call
+ * returns after the copy completed. */
+int cardiac_set_state(cardiac_ctx*, const double* src, int src_on_device);
+
+/* Advance every batch member by nsteps time steps of size dt.  nsteps == 0 is a no-op, nsteps < 0
+ * is invalid.  Asynchronous on the context stream. */
+int cardiac_step(cardiac_ctx*, long long nsteps);
+
+/* Copy the current state out, layout as in set_state. */
+int cardiac_get_state(cardiac_ctx*, double* dst, int dst_on_device);
+
+/* Finite-difference Jacobian-vector products of the flow map: with member 0 the
+ * base trajectory phi(x) and members b = 1..batch-1 the perturbed ones phi(x + eps v_b), write
+ * J_b = (phi(x + eps v_b) - phi(x)) / eps as dense [batch-1][n_v][ny][nx] float64 into dst. */
+int cardiac_get_jvp(cardiac_ctx*, double eps, double* dst, int dst_on_device);
+
+/* Total number of kernels this context has launched (graph nodes counted per replay). */
+long long cardiac_launch_count(const cardiac_ctx*);
+
+/* Run `nsteps` steps `reps` times back to back on the context stream and return, via CUDA events
+ * recorded on that stream, the device time in milliseconds of the whole run in *ms_total
+ * (synchronises the stream).  Used by bench.py for the live per-launch timing of the roofline. */
+int cardiac_time_steps(cardiac_ctx*, long long nsteps, int reps, float* ms_total);
+
+/* Text of the last error on this context; ctx == NULL: the calling thread's last create() error.
+ * Never NULL; empty string when there was none. */
+const char* cardiac_last_error(const cardiac_ctx*);
+
+void cardiac_destroy(cardiac_ctx*);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CARDIAC_H */

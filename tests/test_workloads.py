@@ -1,0 +1,68 @@
+"""Host logic of the seeded input generators (no GPU, no oracle arithmetic)."""
+import numpy as np
+import pytest
+
+from paper_1309_1720_b200 import workloads as W
+
+
+def test_rng_is_counter_based_and_reproducible():
+    a = W.uniform01(3, 1000)
+    assert np.array_equal(a, W.uniform01(3, 1000))
+    assert np.array_equal(a[:100], W.uniform01(3, 100))         # independent of how many are drawn
+    assert not np.array_equal(a, W.uniform01(4, 1000))
+    assert not np.array_equal(a, W.uniform01(3, 1000, stream=1))
+    assert a.min() >= 0.0 and a.max() < 1.0 and abs(a.mean() - 0.5) < 0.05
+    g = W.gaussian(9, 200_000)
+    assert abs(g.mean()) < 0.01 and abs(g.std() - 1.0) < 0.01
+
+
+def test_baseline_configs_follow_baseline_json():
+    c = [W.baseline_config(i) for i in range(1, 6)]
+    assert [(x.model, x.nx, x.ny, x.stencil, x.integrator, x.nsteps, x.batch) for x in c] == [
+        (W.FHN, 64, 64, W.LAP5, W.EULER, 200, 1),
+        (W.FHN, 512, 512, W.LAP9X4, W.RK4, 10_000, 1),
+        (W.KARMA, 1024, 1024, W.LAP5, W.RK4, 5_000, 1),
+        (W.BOCF, 2048, 2048, W.LAP9X4, W.RK4, 2_000, 1),
+        (W.FHN, 512, 512, W.LAP9X4, W.RK4, 1_000, 17)]
+    # dt = 0.5 * dx^2 / (4 D_max)  (BASELINE.json:configs[0])
+    assert c[0].dt == pytest.approx(0.5 * 0.04 ** 2 / (4 * 1.5), rel=1e-15)
+    assert c[2].dt == pytest.approx(0.0780045454545, rel=1e-9)
+    assert c[3].dt == pytest.approx(0.0960717335611, rel=1e-9)
+    assert c[1].scheme == 1 | (2 << 8)
+    with pytest.raises(ValueError):
+        W.baseline_config(6)
+
+
+def test_initial_states():
+    c1 = W.baseline_config(1)
+    z = W.initial_state(c1)
+    assert z.shape == (1, 2, 64, 64) and z.dtype == np.float64
+    assert np.all(np.abs(z[0, 0, :, :5] - 1.0) <= 1e-3) and np.all(np.abs(z[0, 0, :, 5:] - W.REST[W.FHN][0]) <= 1e-3)
+    assert np.all(np.abs(z[0, 1] - W.REST[W.FHN][1]) <= 1e-3) and z[0, 1].std() > 1e-4
+    assert np.array_equal(z, W.initial_state(c1))
+
+    c2 = W.scaled(W.baseline_config(2), 32)
+    z = W.initial_state(c2)[0]
+    assert np.allclose(z[0, :16, :16], 1.0, atol=1e-5) and np.allclose(z[0, 16:, :], W.REST[W.FHN][0], atol=1e-5)
+    assert np.allclose(z[1, 16:, :], 0.0219, atol=1e-3) and np.allclose(z[1, :16, :], W.REST[W.FHN][1], atol=1e-5)
+
+    c3 = W.scaled(W.baseline_config(3), 48, ny=40)
+    z = W.initial_state(c3)[0]
+    assert z.shape == (2, 40, 48)
+    assert 0.0 <= z[0].min() and z[0].max() <= 3.5 and 0.0 <= z[1].min() and z[1].max() <= 1.0
+    assert np.abs(np.diff(z[0], axis=1)).max() < 1.5      # smoothed: no raw block edges
+
+    c4 = W.scaled(W.baseline_config(4), 32)
+    z = W.initial_state(c4)
+    assert np.all(z[0, 0, :, :8] == 1.0) and np.all(z[0, 0, :, 8:] == 0.0)
+    for f in (1, 2, 3):
+        assert np.all(z[0, f] == W.REST[W.BOCF][f])
+    s = W.stimulus_cfg4(z)
+    assert np.all(s[0, 0, :16, :] == 1.0) and np.array_equal(s[0, 1:], z[0, 1:]) and np.array_equal(s[0, 0, 16:], z[0, 0, 16:])
+
+    c5 = W.scaled(W.baseline_config(5), 24)
+    z = W.initial_state(c5)
+    assert z.shape == (17, 2, 24, 24)
+    d = (z[1:] - z[0]) / 1e-7
+    assert np.allclose(np.sqrt(np.sum(d ** 2, axis=(1, 2, 3))), 1.0, atol=1e-6)
+    assert abs(np.sum(d[0] * d[1])) < 0.2                 # different directions

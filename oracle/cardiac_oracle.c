@@ -24,6 +24,12 @@
 #include <stdlib.h>
 #include <string.h>
 
+#ifdef _OPENMP
+#define OMP_FOR _Pragma("omp parallel for")
+#else
+#define OMP_FOR
+#endif
+
 enum { M_FHN = 0, M_KARMA = 1, M_BOCF = 2 };
 enum { S_LAP5 = 0, S_LAP9X4 = 1, S_BOX9 = 2 };
 enum { I_EULER = 0, I_HEUN = 1, I_RK4 = 2, I_RUSH_LARSEN = 3, I_IMPLICIT_EULER = 4 };
@@ -276,7 +282,10 @@ static void rhs(const problem* q, const double* Z, double* F, double* lapbuf) {
   for (int f = 0; f < q->nd; ++f) {
     double D = (q->model == M_FHN) ? q->p[f] : q->p[0];
     oracle_laplacian(Z + f * n, lapbuf, q->nx, q->ny, q->dx, q->stencil, q->boundary);
-    for (size_t c = 0; c < n; ++c) F[f * n + c] = D * lapbuf[c];
+#ifdef _OPENMP
+#pragma omp parallel for
+#endif
+    for (long c = 0; c < (long)n; ++c) F[f * n + c] = D * lapbuf[c];
   }
   for (int f = q->nd; f < q->nv; ++f)
     for (size_t c = 0; c < n; ++c) F[f * n + c] = 0.0;
@@ -320,23 +329,30 @@ static void step_once(const problem* q, double* Z, double* w) {
   if (q->integrator == I_EULER) {
     /* PAPER.md:118; z+ = z + dt f(z) */
     rhs(q, Z, K1, lapbuf);
-    for (size_t c = 0; c < N; ++c) Z[c] = Z[c] + dt * K1[c];
+    OMP_FOR
+    for (long c = 0; c < (long)N; ++c) Z[c] = Z[c] + dt * K1[c];
   } else if (q->integrator == I_HEUN) {
     /* PAPER.md:118, :132, Fig. 2; explicit trapezoid (Q12) */
     rhs(q, Z, K1, lapbuf);
-    for (size_t c = 0; c < N; ++c) Y[c] = Z[c] + dt * K1[c];
+    OMP_FOR
+    for (long c = 0; c < (long)N; ++c) Y[c] = Z[c] + dt * K1[c];
     rhs(q, Y, K2, lapbuf);
-    for (size_t c = 0; c < N; ++c) Z[c] = Z[c] + (dt / 2.0) * (K1[c] + K2[c]);
+    OMP_FOR
+    for (long c = 0; c < (long)N; ++c) Z[c] = Z[c] + (dt / 2.0) * (K1[c] + K2[c]);
   } else if (q->integrator == I_RK4) {
     /* PAPER.md:118 "classic Runge-Kutta" */
     rhs(q, Z, K1, lapbuf);
-    for (size_t c = 0; c < N; ++c) Y[c] = Z[c] + (dt / 2.0) * K1[c];
+    OMP_FOR
+    for (long c = 0; c < (long)N; ++c) Y[c] = Z[c] + (dt / 2.0) * K1[c];
     rhs(q, Y, K2, lapbuf);
-    for (size_t c = 0; c < N; ++c) Y[c] = Z[c] + (dt / 2.0) * K2[c];
+    OMP_FOR
+    for (long c = 0; c < (long)N; ++c) Y[c] = Z[c] + (dt / 2.0) * K2[c];
     rhs(q, Y, K3, lapbuf);
-    for (size_t c = 0; c < N; ++c) Y[c] = Z[c] + dt * K3[c];
+    OMP_FOR
+    for (long c = 0; c < (long)N; ++c) Y[c] = Z[c] + dt * K3[c];
     rhs(q, Y, K4, lapbuf);
-    for (size_t c = 0; c < N; ++c)
+    OMP_FOR
+    for (long c = 0; c < (long)N; ++c)
       Z[c] = Z[c] + (dt / 6.0) * (K1[c] + 2.0 * K2[c] + 2.0 * K3[c] + K4[c]);
   } else {
     /* BOCF only: u by explicit Euler; the non-diffusive variables
@@ -397,6 +413,7 @@ int oracle_step(int model, int nx, int ny, double dx, double dt, int scheme, int
 int oracle_jvp(const double* Z, int batch, size_t N, double eps, double* J) {
   if (batch < 2 || !(eps != 0.0)) return -1;
   for (int b = 1; b < batch; ++b)
-    for (size_t c = 0; c < N; ++c) J[(size_t)(b - 1) * N + c] = (Z[(size_t)b * N + c] - Z[c]) / eps;
+    OMP_FOR
+    for (long c = 0; c < (long)N; ++c) J[(size_t)(b - 1) * N + c] = (Z[(size_t)b * N + c] - Z[c]) / eps;
   return 0;
 }

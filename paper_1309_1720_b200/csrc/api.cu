@@ -1,0 +1,432 @@
+// api.cu — the C ABI of include/cardiac.h: context, validation, workspace, plan selection,
+// CUDA-graph capture of the per-step launch sequence, state copies.  No arithmetic of the method
+// lives here; it only sequences the kernels of *_kernels.cu.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/cardiac.h"
+#include "plans.h"
+#include "stage.cuh"
+
+using namespace cardiac;
+
+namespace {
+thread_local std::string g_create_error;
+
+constexpr int kMaxBuf = 4;
+constexpr int kGraphNodes = 64;  // kernel nodes per captured graph
+}  // namespace
+
+struct cardiac_ctx {
+  Problem pb{};
+  int scheme = 0;
+  int nparams = 0;
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  cudaStream_t cap_stream = nullptr;  // only ever used in capture mode
+  int plan_req = CARDIAC_PLAN_AUTO, plan = CARDIAC_PLAN_STAGE, plan_param = 0;
+  void* ws = nullptr;
+  size_t ws_bytes = 0;
+  bool ws_owned = false;
+  int nbuf = 0;
+  double* buf[kMaxBuf] = {nullptr, nullptr, nullptr, nullptr};
+  int cur = 0;  // buffer holding the state
+  bool has_state = false;
+  cudaGraphExec_t graph[2] = {nullptr, nullptr};  // keyed by `cur` parity at graph start
+  int graph_steps = 0;
+  long long launches = 0;
+  std::string err;
+};
+
+namespace {
+
+int fail(cardiac_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg;
+  return code;
+}
+int fail_cuda(cardiac_ctx* c, cudaError_t e, const char* what) {
+  return fail(c, CARDIAC_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CK(call)                                                  \
+  do {                                                            \
+    cudaError_t e_ = (call);                                      \
+    if (e_ != cudaSuccess) return fail_cuda(c, e_, #call);        \
+  } while (0)
+
+int stages_of(int integ) { return integ == I_HEUN ? 2 : (integ == I_RK4 ? 4 : 1); }
+int buffers_of(int integ) { return integ == I_RK4 ? 4 : 2; }
+
+size_t buffer_doubles(const Problem& pb) { return (size_t)pb.bstride * pb.batch; }
+
+void drop_graphs(cardiac_ctx* c) {
+  for (auto& g : c->graph)
+    if (g) { cudaGraphExecDestroy(g); g = nullptr; }
+  c->graph_steps = 0;
+}
+
+void carve(cardiac_ctx* c) {
+  size_t n = buffer_doubles(c->pb);
+  for (int b = 0; b < c->nbuf; ++b) c->buf[b] = (double*)c->ws + b * n;
+}
+
+// Enqueue the kernels of ONE time step on `s`; advances c->cur as the real execution would.
+int enqueue_step(cardiac_ctx* c, cudaStream_t s) {
+  const Problem& pb = c->pb;
+  const double dt = pb.dt;
+  StageLaunch st{};
+  auto go = [&](int kind, const double* in, const double* y, const double* A, const double* B,
+                double* out, double w_y, double w_in, double w_A, double w_B, double w_f) -> int {
+    st.kind = kind; st.in = in; st.y = y; st.A = A; st.B = B; st.out = out;
+    st.w_y = w_y; st.w_in = w_in; st.w_A = w_A; st.w_B = w_B; st.w_f = w_f;
+    cudaError_t e = launch_stage(pb, st, s);
+    if (e != cudaSuccess) return fail_cuda(c, e, "stage launch");
+    c->launches++;
+    return CARDIAC_OK;
+  };
+  int rc = CARDIAC_OK;
+  double** b = c->buf;
+  switch (pb.integrator) {
+    case I_EULER:
+    case I_RUSH_LARSEN:
+    case I_IMPLICIT_EULER: {
+      int kind = pb.integrator == I_EULER ? K_SELF : (pb.integrator == I_RUSH_LARSEN ? K_RL : K_IE);
+      rc = go(kind, b[c->cur], nullptr, nullptr, nullptr, b[1 - c->cur], 0, 0, 0, 0, dt);
+      c->cur ^= 1;
+      break;
+    }
+    case I_HEUN:
+      // Y2 = y + dt f(y);  y+ = (y + Y2)/2 + dt/2 f(Y2)   [= y + dt/2 (f(y) + f(Y2))]
+      if ((rc = go(K_SELF, b[0], nullptr, nullptr, nullptr, b[1], 0, 0, 0, 0, dt))) break;
+      rc = go(K_BASE, b[1], b[0], nullptr, nullptr, b[0], 0.5, 0.5, 0, 0, 0.5 * dt);
+      break;
+    case I_RK4:
+      // Y2 = y + dt/2 f(y); Y3 = y + dt/2 f(Y2); Y4 = y + dt f(Y3);
+      // y+ = (Y2 + 2 Y3 + Y4 - y)/3 + dt/6 f(Y4)   [accumulator-free classic RK4]
+      if ((rc = go(K_SELF, b[0], nullptr, nullptr, nullptr, b[1], 0, 0, 0, 0, 0.5 * dt))) break;
+      if ((rc = go(K_BASE, b[1], b[0], nullptr, nullptr, b[2], 1.0, 0.0, 0, 0, 0.5 * dt))) break;
+      if ((rc = go(K_BASE, b[2], b[0], nullptr, nullptr, b[3], 1.0, 0.0, 0, 0, dt))) break;
+      rc = go(K_RK4F, b[3], b[0], b[1], b[2], b[0], -1.0 / 3.0, 1.0 / 3.0, 1.0 / 3.0, 2.0 / 3.0,
+              dt / 6.0);
+      break;
+    default:
+      rc = fail(c, CARDIAC_ERR_INVALID, "unknown integrator");
+  }
+  return rc;
+}
+
+// Capture `steps` time steps starting from parity `cur` into an executable graph.
+int build_graph(cardiac_ctx* c, int steps) {
+  int parity = c->cur;
+  long long launches_before = c->launches;
+  CK(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
+  int rc = CARDIAC_OK;
+  for (int s = 0; s < steps && rc == CARDIAC_OK; ++s) rc = enqueue_step(c, c->cap_stream);
+  cudaGraph_t g = nullptr;
+  cudaError_t e = cudaStreamEndCapture(c->cap_stream, &g);
+  c->cur = parity;  // capture executed nothing
+  c->launches = launches_before;
+  if (rc != CARDIAC_OK) { if (g) cudaGraphDestroy(g); return rc; }
+  if (e != cudaSuccess) return fail_cuda(c, e, "cudaStreamEndCapture");
+  e = cudaGraphInstantiate(&c->graph[parity], g, 0);
+  cudaGraphDestroy(g);
+  if (e != cudaSuccess) return fail_cuda(c, e, "cudaGraphInstantiate");
+  c->graph_steps = steps;
+  return CARDIAC_OK;
+}
+
+int ensure_workspace(cardiac_ctx* c) {
+  if (c->ws) return CARDIAC_OK;
+  size_t bytes = cardiac_workspace_bytes(c);
+  CK(cudaMalloc(&c->ws, bytes));
+  c->ws_bytes = bytes;
+  c->ws_owned = true;
+  carve(c);
+  return CARDIAC_OK;
+}
+
+struct DeviceGuard {
+  int prev = -1;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+    if (prev != dev) cudaSetDevice(dev);
+    else prev = -1;
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+}  // namespace
+
+extern "C" {
+
+int cardiac_num_fields(int model) {
+  switch (model) {
+    case CARDIAC_FHN: return 2;
+    case CARDIAC_KARMA: return 2;
+    case CARDIAC_BOCF: return 4;
+  }
+  return -1;
+}
+
+int cardiac_num_params(int model) {
+  switch (model) {
+    case CARDIAC_FHN: return 5;
+    case CARDIAC_KARMA: return 9;
+    case CARDIAC_BOCF: return 30;
+  }
+  return -1;
+}
+
+int cardiac_default_params(int model, double* p, int n) {
+  if (!p || n != cardiac_num_params(model)) return CARDIAC_ERR_INVALID;
+  // FHN: PAPER.md:54.  Karma: PAPER.md:63 + Ref. [2] values (Q7).  BOCF: PAPER.md:76,
+  // epicardial set of Ref. [3] (Q9), D in cm^2/ms.  k = 28.4: PAPER.md:96.
+  static const double fhn[5] = {1.0, 1.5, 0.05, 1.5, -0.1};
+  static const double karma[9] = {0.0011, 2.5, 250.0, 3.0, 1.0, 1.5415, 1.0, 6.0, 28.4};
+  static const double bocf[30] = {1.171e-3, 28.4,   0.0,    1.55,   0.3,    0.13,    0.006,  0.006,
+                                  60.0,     1150.0, 1.4506, 60.0,   15.0,   65.0,    0.03,   200.0,
+                                  0.11,     400.0,  6.0,    30.0181, 0.9957, 2.0458, 0.65,   2.7342,
+                                  16.0,     2.0994, 0.9087, 1.8875, 0.07,   0.94};
+  const double* src = model == CARDIAC_FHN ? fhn : (model == CARDIAC_KARMA ? karma : bocf);
+  std::memcpy(p, src, sizeof(double) * n);
+  return CARDIAC_OK;
+}
+
+cardiac_ctx* cardiac_create(int model, int nx, int ny, double dx, double dt, int scheme, int batch) {
+  auto bad = [](const std::string& m) -> cardiac_ctx* { g_create_error = m; return nullptr; };
+  g_create_error.clear();
+  const int nv = cardiac_num_fields(model);
+  if (nv < 0) return bad("unknown model");
+  const int stencil = scheme & 0xff, integ = (scheme >> 8) & 0xff, bc = (scheme >> 16) & 0xff,
+            variant = (scheme >> 24) & 0xff;
+  if (scheme < 0 || stencil > S_BOX9) return bad("unknown stencil bits");
+  if (integ > I_IMPLICIT_EULER) return bad("unknown integrator bits");
+  if (bc > B_PERIODIC) return bad("unknown boundary bits");
+  if (variant > V_TANHFREE) return bad("unknown variant bits");
+  if (integ >= I_RUSH_LARSEN && model != CARDIAC_BOCF)
+    return bad("Rush-Larsen / implicit Euler are defined for the BOCF gates only");
+  const int r = stencil_radius(stencil);
+  if (nx < 2 * r + 1 || ny < 2 * r + 1) return bad("nx, ny must be >= 2*radius+1");
+  if (nx > (1 << 20) || ny > (1 << 20)) return bad("nx, ny too large");
+  if (batch < 1 || batch > 65535) return bad("batch must be in [1, 65535]");
+  if (!(dx > 0.0) || !std::isfinite(dx)) return bad("dx must be finite and > 0");
+  if (!(dt > 0.0) || !std::isfinite(dt)) return bad("dt must be finite and > 0");
+
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return bad(std::string("no CUDA device: ") + cudaGetErrorString(e));
+  cudaDeviceProp prop{};
+  e = cudaGetDeviceProperties(&prop, dev);
+  if (e != cudaSuccess) return bad(std::string("cudaGetDeviceProperties: ") + cudaGetErrorString(e));
+  if (prop.major != 10)
+    return bad("libcardiac is built for sm_100a (B200) only; found compute capability " +
+               std::to_string(prop.major) + "." + std::to_string(prop.minor));
+
+  cardiac_ctx* c = new (std::nothrow) cardiac_ctx();
+  if (!c) return bad("out of host memory");
+  Problem& pb = c->pb;
+  pb.model = model; pb.stencil = stencil; pb.integrator = integ; pb.boundary = bc;
+  pb.variant = variant; pb.nx = nx; pb.ny = ny; pb.batch = batch; pb.nv = nv;
+  pb.nd = model == CARDIAC_FHN ? 2 : 1; pb.radius = r;
+  pb.pitch = (nx + 15) / 16 * 16;
+  pb.fstride = (long long)pb.pitch * ny;
+  pb.bstride = pb.fstride * nv;
+  pb.dx = dx; pb.dt = dt;
+  c->scheme = scheme;
+  c->nparams = cardiac_num_params(model);
+  cardiac_default_params(model, pb.params, c->nparams);
+  c->device = dev;
+  c->nbuf = buffers_of(integ);
+  e = cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking);
+  if (e != cudaSuccess) {
+    delete c;
+    return bad(std::string("cudaStreamCreate: ") + cudaGetErrorString(e));
+  }
+  return c;
+}
+
+int cardiac_set_params(cardiac_ctx* c, const double* p, int n) {
+  if (!c) return CARDIAC_ERR_INVALID;
+  if (!p || n != c->nparams) return fail(c, CARDIAC_ERR_INVALID, "wrong parameter count");
+  for (int i = 0; i < n; ++i)
+    if (!std::isfinite(p[i])) return fail(c, CARDIAC_ERR_INVALID, "non-finite parameter");
+  if (c->pb.model == CARDIAC_KARMA) {
+    double M = p[7];
+    if (M != std::floor(M) || M < 1 || M > 16)
+      return fail(c, CARDIAC_ERR_INVALID, "Karma M must be an integer in [1,16]");
+  }
+  std::memcpy(c->pb.params, p, sizeof(double) * n);
+  drop_graphs(c);
+  return CARDIAC_OK;
+}
+
+int cardiac_get_params(const cardiac_ctx* c, double* p, int n) {
+  if (!c || !p || n != c->nparams) return CARDIAC_ERR_INVALID;
+  std::memcpy(p, c->pb.params, sizeof(double) * n);
+  return CARDIAC_OK;
+}
+
+int cardiac_set_stream(cardiac_ctx* c, void* cuda_stream) {
+  if (!c) return CARDIAC_ERR_INVALID;
+  c->stream = (cudaStream_t)cuda_stream;
+  return CARDIAC_OK;
+}
+
+int cardiac_set_plan(cardiac_ctx* c, int plan, int param) {
+  if (!c) return CARDIAC_ERR_INVALID;
+  if (plan != CARDIAC_PLAN_AUTO && plan != CARDIAC_PLAN_STAGE)
+    return fail(c, CARDIAC_ERR_INVALID, "plan not available for this context");
+  if (param != 0) return fail(c, CARDIAC_ERR_INVALID, "plan parameter must be 0");
+  c->plan_req = plan;
+  c->plan = CARDIAC_PLAN_STAGE;
+  c->plan_param = param;
+  drop_graphs(c);
+  return CARDIAC_OK;
+}
+
+int cardiac_get_plan(const cardiac_ctx* c) { return c ? c->plan : CARDIAC_ERR_INVALID; }
+
+size_t cardiac_workspace_bytes(const cardiac_ctx* c) {
+  if (!c) return 0;
+  return buffer_doubles(c->pb) * sizeof(double) * c->nbuf;
+}
+
+int cardiac_bind_workspace(cardiac_ctx* c, void* dev_ptr, size_t bytes) {
+  if (!c) return CARDIAC_ERR_INVALID;
+  if (c->ws) return fail(c, CARDIAC_ERR_INVALID, "workspace already bound");
+  if (!dev_ptr) return fail(c, CARDIAC_ERR_INVALID, "null workspace");
+  if (bytes < cardiac_workspace_bytes(c) || ((size_t)dev_ptr & 255))
+    return fail(c, CARDIAC_ERR_WORKSPACE, "workspace too small or not 256-byte aligned");
+  c->ws = dev_ptr;
+  c->ws_bytes = bytes;
+  c->ws_owned = false;
+  carve(c);
+  return CARDIAC_OK;
+}
+
+int cardiac_set_state(cardiac_ctx* c, const double* src, int src_on_device) {
+  if (!c) return CARDIAC_ERR_INVALID;
+  if (!src) return fail(c, CARDIAC_ERR_INVALID, "null source");
+  DeviceGuard guard(c->device);
+  int rc = ensure_workspace(c);
+  if (rc) return rc;
+  const Problem& pb = c->pb;
+  c->cur = 0;
+  CK(cudaMemcpy2DAsync(c->buf[0], (size_t)pb.pitch * sizeof(double), src,
+                       (size_t)pb.nx * sizeof(double), (size_t)pb.nx * sizeof(double),
+                       (size_t)pb.ny * pb.nv * pb.batch,
+                       src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+  if (!src_on_device) CK(cudaStreamSynchronize(c->stream));
+  c->has_state = true;
+  return CARDIAC_OK;
+}
+
+int cardiac_get_state(cardiac_ctx* c, double* dst, int dst_on_device) {
+  if (!c) return CARDIAC_ERR_INVALID;
+  if (!dst) return fail(c, CARDIAC_ERR_INVALID, "null destination");
+  if (!c->has_state) return fail(c, CARDIAC_ERR_NOSTATE, "no state set");
+  DeviceGuard guard(c->device);
+  const Problem& pb = c->pb;
+  CK(cudaMemcpy2DAsync(dst, (size_t)pb.nx * sizeof(double), c->buf[c->cur],
+                       (size_t)pb.pitch * sizeof(double), (size_t)pb.nx * sizeof(double),
+                       (size_t)pb.ny * pb.nv * pb.batch,
+                       dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
+  if (!dst_on_device) CK(cudaStreamSynchronize(c->stream));
+  return CARDIAC_OK;
+}
+
+int cardiac_step(cardiac_ctx* c, long long nsteps) {
+  if (!c) return CARDIAC_ERR_INVALID;
+  if (nsteps < 0) return fail(c, CARDIAC_ERR_INVALID, "nsteps < 0");
+  if (!c->has_state) return fail(c, CARDIAC_ERR_NOSTATE, "no state set");
+  if (nsteps == 0) return CARDIAC_OK;
+  DeviceGuard guard(c->device);
+  const int ns = stages_of(c->pb.integrator);
+  int gsteps = kGraphNodes / ns;
+  if (gsteps & 1) gsteps++;  // even: ping-pong integrators end on the parity they started on
+  long long left = nsteps;
+  if (left >= gsteps) {
+    if (c->graph_steps != gsteps) drop_graphs(c);
+    if (!c->graph[c->cur]) {
+      int rc = build_graph(c, gsteps);
+      if (rc) return rc;
+    }
+    while (left >= gsteps) {
+      CK(cudaGraphLaunch(c->graph[c->cur], c->stream));
+      c->launches += (long long)gsteps * ns;
+      left -= gsteps;
+    }
+  }
+  for (; left > 0; --left) {
+    int rc = enqueue_step(c, c->stream);
+    if (rc) return rc;
+  }
+  return CARDIAC_OK;
+}
+
+int cardiac_get_jvp(cardiac_ctx* c, double eps, double* dst, int dst_on_device) {
+  if (!c) return CARDIAC_ERR_INVALID;
+  if (!dst) return fail(c, CARDIAC_ERR_INVALID, "null destination");
+  if (!c->has_state) return fail(c, CARDIAC_ERR_NOSTATE, "no state set");
+  if (c->pb.batch < 2) return fail(c, CARDIAC_ERR_INVALID, "JVP needs batch >= 2");
+  if (!(eps != 0.0) || !std::isfinite(eps)) return fail(c, CARDIAC_ERR_INVALID, "bad eps");
+  DeviceGuard guard(c->device);
+  const Problem& pb = c->pb;
+  if (dst_on_device) {
+    cudaError_t e = launch_jvp(pb, c->buf[c->cur], eps, dst, c->stream);
+    if (e != cudaSuccess) return fail_cuda(c, e, "jvp launch");
+    c->launches++;
+    return CARDIAC_OK;
+  }
+  size_t bytes = (size_t)pb.nx * pb.ny * pb.nv * (pb.batch - 1) * sizeof(double);
+  double* tmp = nullptr;
+  CK(cudaMalloc(&tmp, bytes));
+  cudaError_t e = launch_jvp(pb, c->buf[c->cur], eps, tmp, c->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(dst, tmp, bytes, cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  cudaFree(tmp);
+  if (e != cudaSuccess) return fail_cuda(c, e, "jvp");
+  c->launches++;
+  return CARDIAC_OK;
+}
+
+long long cardiac_launch_count(const cardiac_ctx* c) { return c ? c->launches : 0; }
+
+int cardiac_time_steps(cardiac_ctx* c, long long nsteps, int reps, float* ms_total) {
+  if (!c) return CARDIAC_ERR_INVALID;
+  if (!ms_total || reps < 1) return fail(c, CARDIAC_ERR_INVALID, "bad arguments");
+  DeviceGuard guard(c->device);
+  cudaEvent_t e0, e1;
+  CK(cudaEventCreate(&e0));
+  CK(cudaEventCreate(&e1));
+  int rc = CARDIAC_OK;
+  cudaError_t e = cudaEventRecord(e0, c->stream);
+  for (int r = 0; r < reps && rc == CARDIAC_OK && e == cudaSuccess; ++r) rc = cardiac_step(c, nsteps);
+  if (e == cudaSuccess) e = cudaEventRecord(e1, c->stream);
+  if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+  if (e == cudaSuccess) e = cudaEventElapsedTime(ms_total, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (rc) return rc;
+  if (e != cudaSuccess) return fail_cuda(c, e, "timing");
+  return CARDIAC_OK;
+}
+
+const char* cardiac_last_error(const cardiac_ctx* c) {
+  return c ? c->err.c_str() : g_create_error.c_str();
+}
+
+void cardiac_destroy(cardiac_ctx* c) {
+  if (!c) return;
+  DeviceGuard guard(c->device);
+  drop_graphs(c);
+  if (c->ws_owned && c->ws) cudaFree(c->ws);
+  if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+  delete c;
+}
+
+}  // extern "C"

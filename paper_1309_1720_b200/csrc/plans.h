@@ -1,0 +1,36 @@
+// plans.h — host-side interface between the C-ABI (api.cu) and the kernel files.  Plain structs,
+// no templates: each *_kernels.cu instantiates its kernels and exports one launcher.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace cardiac {
+
+struct Problem {
+  int model, stencil, integrator, boundary, variant;
+  int nx, ny, batch, nv, nd, radius;
+  int pitch;            // doubles per row
+  long long fstride;    // doubles per field
+  long long bstride;    // doubles per batch member
+  double dx, dt;
+  double params[32];    // public parameter block (include/cardiac.h)
+};
+
+// One stage launch of the STAGE plan (kind = K_* of stage.cuh).
+struct StageLaunch {
+  int kind;
+  const double* in;
+  const double* y;
+  const double* A;
+  const double* B;
+  double* out;
+  double w_y, w_in, w_A, w_B, w_f;
+};
+
+// stage_kernels.cu: fused stencil + reaction + RK-stage combine, one launch per substep.
+cudaError_t launch_stage(const Problem& pb, const StageLaunch& st, cudaStream_t stream);
+
+// jvp: J[b-1] = (Z[b] - Z[0]) / eps, pitched state -> dense output
+cudaError_t launch_jvp(const Problem& pb, const double* state, double eps, double* dst_dense,
+                       cudaStream_t stream);
+
+}  // namespace cardiac

@@ -1,0 +1,92 @@
+// stage.cuh — argument blocks and the Laplacian weights shared by all execution plans.
+#pragma once
+#include "models.cuh"
+
+namespace cardiac {
+
+enum { S_LAP5 = 0, S_LAP9X4 = 1, S_BOX9 = 2 };
+enum { B_NOFLUX = 0, B_PERIODIC = 1 };
+enum { I_EULER = 0, I_HEUN = 1, I_RK4 = 2, I_RUSH_LARSEN = 3, I_IMPLICIT_EULER = 4 };
+
+// What one stage launch writes (every RK substep is "some combination of local, non-local and
+// Euler-like update"):
+//   K_SELF : out = in + w_f f(in)                                     Euler; Heun/RK4 stage 1
+//   K_BASE : out = w_y y + w_in in + w_f f(in)                         RK4 stages 2,3; Heun stage 2
+//   K_RK4F : out = w_y y + w_A A + w_B B + w_in in + w_f f(in)         RK4 stage 4, accumulator-free:
+//            y+ = (Y2 + 2 Y3 + Y4 - y)/3 + dt/6 f(Y4)
+//   K_RL / K_IE : BOCF, u by Euler, gates by Rush-Larsen / implicit Euler
+enum { K_SELF = 0, K_BASE = 1, K_RK4F = 2, K_RL = 3, K_IE = 4 };
+
+__host__ __device__ constexpr int stencil_radius(int stencil) { return stencil == S_LAP9X4 ? 2 : 1; }
+// lap(U) = lap_norm * (integer-weight stencil sum) / dx^2
+__host__ __device__ constexpr double stencil_norm(int stencil) {
+  return stencil == S_LAP9X4 ? 1.0 / 12.0 : (stencil == S_BOX9 ? 1.0 / 6.0 : 1.0);
+}
+
+// State buffers are [batch][n_v][ny] rows of `pitch` doubles (pitch >= nx, multiple of 16 so every
+// row starts 128-byte aligned); x fastest.
+struct Geom {
+  int nx, ny, pitch, boundary;
+  long long fstride;  // doubles between fields  (= pitch * ny)
+  long long bstride;  // doubles between batch members (= fstride * n_v)
+};
+
+template <class MD>
+struct StageArgs {
+  const double* in;  // stage input (read with halo for the diffusing fields)
+  const double* y;   // state at the start of the step (pointwise)
+  const double* A;   // Y2 (pointwise, K_RK4F)
+  const double* B;   // Y3 (pointwise, K_RK4F)
+  double* out;       // may alias y (in-place final stage), never in
+  Geom g;
+  double w_y, w_in, w_A, w_B, w_f;  // w_f already contains dt
+  double dt;
+  double lapw[MD::ND];  // D_f * stencil_norm / dx^2
+  typename MD::Params p;
+};
+
+// out-of-range index -> in-range index ("flip displacement vectors which cross the
+// domain boundary back into the domain"; index reflection about the boundary node, Q3;
+// periodic: "mapping to the opposite-edge values")
+CARDIAC_D int bidx(int i, int n, int boundary) {
+  if (boundary == B_PERIODIC) return i < 0 ? i + n : (i >= n ? i - n : i);
+  return i < 0 ? -i : (i >= n ? 2 * (n - 1) - i : i);
+}
+
+// integer-weight stencil sums
+template <int STENCIL>
+struct Stencil;
+template <>
+struct Stencil<S_LAP5> {
+  // c, then W, E, S, N
+  CARDIAC_D static double apply(double c, double w, double e, double s, double n) {
+    return fma(-4.0, c, (w + e) + (s + n));
+  }
+};
+template <>
+struct Stencil<S_LAP9X4> {
+  CARDIAC_D static double apply(double c, double w1, double e1, double s1, double n1, double w2,
+                                double e2, double s2, double n2) {
+    double a1 = (w1 + e1) + (s1 + n1), a2 = (w2 + e2) + (s2 + n2);
+    return fma(-60.0, c, fma(16.0, a1, -a2));
+  }
+};
+template <>
+struct Stencil<S_BOX9> {
+  CARDIAC_D static double apply(double c, double w, double e, double s, double n, double sw,
+                                double se, double nw, double ne) {
+    double ax = (w + e) + (s + n), dg = (sw + se) + (nw + ne);
+    return fma(-20.0, c, fma(4.0, ax, dg));
+  }
+};
+
+// the RK combination of one field value, shared by every plan
+template <int KIND>
+CARDIAC_D double combine(double w_y, double w_in, double w_A, double w_B, double w_f, double y,
+                         double in, double A, double B, double f) {
+  if (KIND == K_SELF) return fma(w_f, f, in);
+  if (KIND == K_BASE) return fma(w_f, f, fma(w_in, in, w_y * y));
+  return fma(w_f, f, fma(w_in, in, fma(w_B, B, fma(w_A, A, w_y * y))));
+}
+
+}  // namespace cardiac

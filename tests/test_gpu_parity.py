@@ -1,0 +1,296 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json:north_star's: max-abs <= 1e-12 after one step and
+<= 1e-9 after 100 steps on non-chaotic runs (FMA contraction allowed on the GPU side; the oracle is
+built with -ffp-contract=off).  Needs a B200.
+"""
+import numpy as np
+import pytest
+
+import oracle as O
+from paper_1309_1720_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_1 = 1e-12     # one step
+TOL_100 = 1e-9    # 100 steps
+
+FHN, KARMA, BOCF = W.FHN, W.KARMA, W.BOCF
+LAP5, LAP9X4, BOX9 = W.LAP5, W.LAP9X4, W.BOX9
+EULER, HEUN, RK4, RL, IE = W.EULER, W.HEUN, W.RK4, W.RUSH_LARSEN, W.IMPLICIT_EULER
+
+
+@pytest.fixture(scope="module")
+def C():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_1309_1720_b200 import cardiac
+    return cardiac
+
+
+def gpu_run(C, cfg, Z0, nsteps, plan=0, plan_param=0, params=None, chunks=None):
+    with C.Context.from_config(cfg, plan=plan, plan_param=plan_param, params=params) as ctx:
+        ctx.set_state(np.ascontiguousarray(Z0))
+        for n in (chunks or [nsteps]):
+            ctx.step(n)
+        out = ctx.get_state()
+        assert ctx.launches > 0
+    return out
+
+
+def maxabs(a, b):
+    return float(np.max(np.abs(a - b)))
+
+
+def make(model, nx, ny, stencil, integ, batch=1, seed=11, **kw):
+    cfg = W.make_config("case", model, nx, stencil, integ, 0, batch=batch, seed=seed, ny=ny, **kw)
+    Z = W.initial_state(cfg)
+    return cfg, Z
+
+
+# ----------------------------------------------------------------------------- every model x stencil x integrator
+CASES = [(m, s, i) for m in (FHN, KARMA, BOCF) for s in (LAP5, LAP9X4, BOX9) for i in (EULER, HEUN, RK4)]
+CASES += [(BOCF, s, i) for s in (LAP5, LAP9X4, BOX9) for i in (RL, IE)]
+
+
+@pytest.mark.parametrize("model,stencil,integ", CASES)
+def test_parity_one_and_hundred_steps(C, model, stencil, integ):
+    # 70 x 45: several 32x8 / 64-wide tiles and a ragged tail in both directions, odd pitch padding
+    cfg, Z = make(model, 70, 45, stencil, integ)
+    got1 = gpu_run(C, cfg, Z, 1)
+    ref1 = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 1)
+    assert maxabs(got1, ref1) <= TOL_1
+    got = gpu_run(C, cfg, Z, 100)
+    ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 100)
+    assert np.all(np.isfinite(got))
+    assert maxabs(got, ref) <= TOL_100
+    assert maxabs(got, Z) > 1e-6          # it did move
+
+
+@pytest.mark.parametrize("model,stencil,integ", [(FHN, LAP9X4, RK4), (KARMA, LAP5, RK4), (BOCF, LAP9X4, RK4),
+                                                 (FHN, LAP5, EULER), (BOCF, BOX9, HEUN)])
+def test_parity_periodic_boundary(C, model, stencil, integ):
+    cfg, Z = make(model, 37, 50, stencil, integ, boundary=1)
+    got = gpu_run(C, cfg, Z, 30)
+    ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 30)
+    assert maxabs(got, ref) <= TOL_100
+
+
+@pytest.mark.parametrize("model", [KARMA, BOCF])
+def test_parity_tanhfree_variant(C, model):
+    cfg, Z = make(model, 40, 33, LAP9X4, RK4, variant=1)
+    got = gpu_run(C, cfg, Z, 50)
+    ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 50)
+    assert maxabs(got, ref) <= TOL_100
+    ref_paper = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme & 0xFFFFFF, 50)
+    assert maxabs(ref, ref_paper) > 1e-6   # the variant really is a different model
+
+
+@pytest.mark.parametrize("model,stencil,nx,ny", [(FHN, LAP5, 3, 3), (FHN, LAP9X4, 5, 5), (KARMA, LAP9X4, 5, 64),
+                                                 (BOCF, LAP5, 200, 3), (FHN, BOX9, 3, 17), (KARMA, LAP5, 33, 4)])
+def test_parity_degenerate_sizes(C, model, stencil, nx, ny):
+    """Minimum sizes 2r+1 (every stencil arm reflects) and thin strips."""
+    cfg, Z = make(model, nx, ny, stencil, RK4)
+    got = gpu_run(C, cfg, Z, 20)
+    ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 20)
+    assert maxabs(got, ref) <= TOL_100
+
+
+def test_batch_members_independent_of_position(C):
+    cfg, Z = make(KARMA, 48, 40, LAP5, RK4, batch=5, seed=3)
+    got = gpu_run(C, cfg, Z, 10)
+    ref = O.step(KARMA, Z, cfg.dx, cfg.dt, cfg.scheme, 10)
+    assert maxabs(got, ref) <= TOL_100
+    perm = [3, 0, 4, 2, 1]
+    got_p = gpu_run(C, cfg, Z[perm], 10)
+    assert np.array_equal(got_p, got[perm])                 # bitwise, whatever the slot
+    import dataclasses
+    single = gpu_run(C, dataclasses.replace(cfg, batch=1), Z[2:3], 10)
+    assert np.array_equal(single[0], got[2])
+
+
+@pytest.mark.parametrize("model,integ", [(FHN, EULER), (FHN, RK4), (KARMA, HEUN), (BOCF, RL)])
+def test_step_composition_and_determinism_bitwise(C, model, integ):
+    """step(a); step(b) == step(a+b), graph replay == direct launches, run-to-run identical."""
+    cfg, Z = make(model, 64, 37, LAP9X4, integ)
+    whole = gpu_run(C, cfg, Z, 137)                         # graph chunks + remainder
+    parts = gpu_run(C, cfg, Z, 137, chunks=[1, 70, 3, 63])
+    singles = gpu_run(C, cfg, Z, 137, chunks=[1] * 137)    # never reaches a graph
+    again = gpu_run(C, cfg, Z, 137)
+    assert np.array_equal(whole, parts) and np.array_equal(whole, singles) and np.array_equal(whole, again)
+
+
+def test_uniform_state_and_rest_state(C):
+    """A uniform state stays uniform (to roundoff of the weighted stencil sum) and the rest states
+    are fixed points."""
+    for model in (FHN, KARMA, BOCF):
+        cfg = W.make_config("rest", model, 40, LAP9X4, RK4, 0, ny=24)
+        Z = np.empty((1, cfg.n_v, 24, 40))
+        for f, r in enumerate(W.REST[model]):
+            Z[0, f] = r
+        got = gpu_run(C, cfg, Z, 50)
+        assert maxabs(got, Z) < 1e-13
+    cfg = W.make_config("uni", FHN, 40, LAP9X4, RK4, 0, ny=24)
+    Z = np.empty((1, 2, 24, 40)); Z[0, 0] = 0.8; Z[0, 1] = -0.1
+    got = gpu_run(C, cfg, Z, 50)
+    ref = O.step(FHN, Z, cfg.dx, cfg.dt, cfg.scheme, 50)
+    assert maxabs(got, ref) < 1e-13
+    assert np.ptp(got[0, 0]) < 1e-13 and np.ptp(got[0, 1]) < 1e-13
+
+
+def test_custom_parameters(C):
+    cfg, Z = make(KARMA, 32, 32, LAP5, RK4)
+    p = O.default_params(KARMA)
+    p[0], p[1], p[5], p[7] = 0.002, 3.0, 1.4, 4.0          # gamma, tau_u, u_star, M = 4
+    got = gpu_run(C, cfg, Z, 20, params=p)
+    ref = O.step(KARMA, Z, cfg.dx, cfg.dt, cfg.scheme, 20, params=p)
+    assert maxabs(got, ref) <= TOL_100
+    assert maxabs(ref, O.step(KARMA, Z, cfg.dx, cfg.dt, cfg.scheme, 20)) > 1e-4
+    with C.Context.from_config(cfg) as ctx:
+        C.cardiac_set_params(ctx.ctx, p)
+        assert np.array_equal(C.cardiac_get_params(ctx.ctx, 9), p)
+        p_bad = p.copy(); p_bad[7] = 2.5
+        with pytest.raises(C.CardiacError):
+            C.cardiac_set_params(ctx.ctx, p_bad)
+        with pytest.raises(C.CardiacError):
+            C.cardiac_set_params(ctx.ctx, p[:5])
+
+
+def test_error_paths_and_device_buffers(C):
+    import torch
+    cfg, Z = make(FHN, 40, 30, LAP5, EULER)
+    ctx = C.cardiac_create(cfg.model, cfg.nx, cfg.ny, cfg.dx, cfg.dt, cfg.scheme, 1)
+    try:
+        with pytest.raises(C.CardiacError) as ei:
+            C.cardiac_step(ctx, 1)
+        assert ei.value.code == C.CARDIAC_ERR_NOSTATE
+        out = np.empty_like(Z)
+        with pytest.raises(C.CardiacError) as ei:
+            C.cardiac_get_state(ctx, out)
+        assert ei.value.code == C.CARDIAC_ERR_NOSTATE
+        need = C.cardiac_workspace_bytes(ctx)
+        assert need >= 2 * Z.nbytes
+        small = torch.empty(need // 2, dtype=torch.uint8, device="cuda")
+        with pytest.raises(C.CardiacError) as ei:
+            C.cardiac_bind_workspace(ctx, small.data_ptr(), small.numel())
+        assert ei.value.code == C.CARDIAC_ERR_WORKSPACE
+        # library-allocated workspace, default stream, device-resident src/dst
+        zd = torch.from_numpy(Z).cuda()
+        C.cardiac_set_state(ctx, zd)
+        with pytest.raises(C.CardiacError):
+            C.cardiac_step(ctx, -1)
+        C.cardiac_step(ctx, 0)
+        C.cardiac_step(ctx, 5)
+        od = torch.empty_like(zd)
+        C.cardiac_get_state(ctx, od)
+        torch.cuda.synchronize()
+        ref = O.step(FHN, Z, cfg.dx, cfg.dt, cfg.scheme, 5)
+        assert maxabs(od.cpu().numpy(), ref) <= TOL_100
+        assert C.cardiac_launch_count(ctx) == 5
+        with pytest.raises(C.CardiacError):
+            C.cardiac_set_plan(ctx, 99, 0)
+        with pytest.raises(TypeError):
+            C.cardiac_set_state(ctx, Z.astype(np.float32))
+        ms = C.cardiac_time_steps(ctx, 10, 3)
+        assert ms > 0 and C.cardiac_launch_count(ctx) == 35
+    finally:
+        C.cardiac_destroy(ctx)
+
+
+def test_non_default_stream(C):
+    import torch
+    cfg, Z = make(FHN, 64, 64, LAP9X4, RK4)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        with C.Context.from_config(cfg) as ctx:
+            zd = torch.from_numpy(Z).cuda()
+            ctx.set_state(zd)
+            ctx.step(40)
+            od = torch.empty_like(zd)
+            ctx.get_state(od)
+            s.synchronize()
+    ref = O.step(FHN, Z, cfg.dx, cfg.dt, cfg.scheme, 40)
+    assert maxabs(od.cpu().numpy(), ref) <= TOL_100
+
+
+# ----------------------------------------------------------------------------- the BASELINE configs at full size
+def test_config1_full(C):
+    cfg = W.baseline_config(1)
+    Z = W.initial_state(cfg)
+    got = gpu_run(C, cfg, Z, cfg.nsteps)            # all 200 steps
+    ref = O.step(cfg.model, Z, cfg.dx, cfg.dt, cfg.scheme, cfg.nsteps)
+    assert maxabs(got, ref) <= TOL_100
+    assert maxabs(gpu_run(C, cfg, Z, 1), O.step(cfg.model, Z, cfg.dx, cfg.dt, cfg.scheme, 1)) <= TOL_1
+
+
+@pytest.mark.parametrize("idx,n100,omp", [(2, 100, False), (3, 100, True), (4, 25, True)])
+def test_configs_full_size_step1_and_step100(C, idx, n100, omp):
+    """Full-size grids, in the launch configuration bench.py times; for the large grids the oracle
+    runs its -fopenmp build (independent loops split over threads, bitwise the same numbers), and
+    config 4 (4.2 M cells x 4 fields of the exp-heavy model) stops at 25 steps to bound CPU time."""
+    cfg = W.baseline_config(idx)
+    Z = W.initial_state(cfg)
+    with C.Context.from_config(cfg) as ctx:
+        ctx.set_state(Z)
+        ctx.step(1)
+        got1 = ctx.get_state()
+        ctx.step(n100 - 1)
+        got = ctx.get_state()
+    ref1 = O.step(cfg.model, Z, cfg.dx, cfg.dt, cfg.scheme, 1, omp=omp)
+    assert maxabs(got1, ref1) <= TOL_1
+    ref = O.step(cfg.model, ref1, cfg.dx, cfg.dt, cfg.scheme, n100 - 1, omp=omp)
+    assert maxabs(got, ref) <= TOL_100
+
+
+def test_config4_stimulus_path(C):
+    """step -> get_state -> host edit -> set_state -> step (config 4's cross-field stimulus), scaled."""
+    cfg = W.scaled(W.baseline_config(4), 96, ny=80)
+    Z = W.initial_state(cfg)
+    with C.Context.from_config(cfg) as ctx:
+        ctx.set_state(Z)
+        ctx.step(60)
+        mid = W.stimulus_cfg4(ctx.get_state())
+        ctx.set_state(mid)
+        ctx.step(40)
+        got = ctx.get_state()
+    ref_mid = W.stimulus_cfg4(O.step(BOCF, Z, cfg.dx, cfg.dt, cfg.scheme, 60))
+    ref = O.step(BOCF, ref_mid, cfg.dx, cfg.dt, cfg.scheme, 40)
+    assert maxabs(got, ref) <= TOL_100
+
+
+def test_config5_jvp_full_size(C):
+    """17 x 512^2 in one batched launch; states at the state tolerance, JVPs at 1e-6 absolute
+    (= 1e-13/eps, Q16)."""
+    cfg = W.baseline_config(5)
+    eps = 1e-7
+    Z = W.initial_state(cfg)
+    n = 20
+    with C.Context.from_config(cfg) as ctx:
+        ctx.set_state(Z)
+        ctx.step(n)
+        got = ctx.get_state()
+        J = ctx.get_jvp(eps)
+        import torch
+        Jd = torch.empty(J.shape, dtype=torch.float64, device="cuda")
+        ctx.get_jvp(eps, Jd)
+        torch.cuda.synchronize()
+    assert np.array_equal(Jd.cpu().numpy(), J)
+    ref = O.step(cfg.model, Z, cfg.dx, cfg.dt, cfg.scheme, n, omp=True)
+    assert maxabs(got, ref) <= TOL_100
+    assert np.array_equal(J, (got[1:] - got[0]) / eps)     # exactly the FD quotient of the states
+    Jref = O.jvp(ref, eps)
+    assert maxabs(J, Jref) <= 1e-6
+    assert np.max(np.abs(Jref)) > 1e-4
+
+
+def test_config5_jvp_scaled_100_steps(C):
+    cfg = W.scaled(W.baseline_config(5), 96)
+    eps = 1e-7
+    Z = W.initial_state(cfg)
+    with C.Context.from_config(cfg) as ctx:
+        ctx.set_state(Z)
+        ctx.step(100)
+        got = ctx.get_state()
+        J = ctx.get_jvp(eps)
+    ref = O.step(cfg.model, Z, cfg.dx, cfg.dt, cfg.scheme, 100)
+    assert maxabs(got, ref) <= TOL_100
+    assert maxabs(J, O.jvp(ref, eps)) <= 1e-6

@@ -146,6 +146,16 @@ int cardiac_get_state(cardiac_ctx*, double* dst, int dst_on_device);
  * J_b = (phi(x + eps v_b) - phi(x)) / eps as dense [batch-1][n_v][ny][nx] float64 into dst. */
 int cardiac_get_jvp(cardiac_ctx*, double eps, double* dst, int dst_on_device);
 
+/* Diagnostic (not on the hot path): evaluate device-side building blocks on n sample points held
+ * in device memory, enqueued on the context stream.
+ *   CARDIAC_PROBE_EXP      out[i] = the library's exp(in[i])            (used inside tanh)
+ *   CARDIAC_PROBE_RCP      out[i] = the library's 1/in[i], in[i] > 0    (divisions)
+ *   CARDIAC_PROBE_HK       out[i] = H_k(in[i]), k of the context's model
+ *   CARDIAC_PROBE_REACTION in = [n][n_v] states, out = [n][n_v] reaction terms N[z] of the
+ *                          context's model, variant and parameters */
+enum { CARDIAC_PROBE_EXP = 0, CARDIAC_PROBE_RCP = 1, CARDIAC_PROBE_HK = 2, CARDIAC_PROBE_REACTION = 3 };
+int cardiac_probe(cardiac_ctx*, int what, const double* in_dev, double* out_dev, long long n);
+
 /* Total number of kernels this context has launched (graph nodes counted per replay). */
 long long cardiac_launch_count(const cardiac_ctx*);
 

@@ -26,13 +26,14 @@ CARDIAC_RUSH_LARSEN, CARDIAC_IMPLICIT_EULER = 3 << 8, 4 << 8
 CARDIAC_NOFLUX, CARDIAC_PERIODIC = 0 << 16, 1 << 16
 CARDIAC_VARIANT_PAPER, CARDIAC_VARIANT_TANHFREE = 0 << 24, 1 << 24
 CARDIAC_PLAN_AUTO, CARDIAC_PLAN_STAGE, CARDIAC_PLAN_FUSED, CARDIAC_PLAN_PERSISTENT = 0, 1, 2, 3
+CARDIAC_PROBE_EXP, CARDIAC_PROBE_RCP, CARDIAC_PROBE_HK, CARDIAC_PROBE_REACTION = 0, 1, 2, 3
 CARDIAC_OK, CARDIAC_ERR_INVALID, CARDIAC_ERR_CUDA, CARDIAC_ERR_NOSTATE, CARDIAC_ERR_WORKSPACE = 0, -1, -2, -3, -4
 
 EXPORTS = [
     "cardiac_num_fields", "cardiac_num_params", "cardiac_default_params", "cardiac_create",
     "cardiac_set_params", "cardiac_get_params", "cardiac_set_stream", "cardiac_set_plan",
     "cardiac_get_plan", "cardiac_workspace_bytes", "cardiac_bind_workspace", "cardiac_set_state",
-    "cardiac_step", "cardiac_get_state", "cardiac_get_jvp", "cardiac_launch_count",
+    "cardiac_step", "cardiac_get_state", "cardiac_get_jvp", "cardiac_probe", "cardiac_launch_count",
     "cardiac_time_steps", "cardiac_last_error", "cardiac_destroy",
 ]
 
@@ -65,6 +66,7 @@ _sig = {
     "cardiac_step": (_i, [_vp, _ll]),
     "cardiac_get_state": (_i, [_vp, _vp, _i]),
     "cardiac_get_jvp": (_i, [_vp, _d, _vp, _i]),
+    "cardiac_probe": (_i, [_vp, _i, _vp, _vp, _ll]),
     "cardiac_launch_count": (_ll, [_vp]),
     "cardiac_time_steps": (_i, [_vp, _ll, _i, ctypes.POINTER(ctypes.c_float)]),
     "cardiac_last_error": (ctypes.c_char_p, [_vp]),
@@ -169,6 +171,14 @@ def cardiac_get_state(ctx, dst) -> None:
 def cardiac_get_jvp(ctx, eps: float, dst) -> None:
     addr, dev, _keep = _buffer(dst)
     _check(ctx, _lib.cardiac_get_jvp(ctx, eps, addr, dev))
+
+
+def cardiac_probe(ctx, what: int, src, dst, n: int) -> None:
+    a, da, _k1 = _buffer(src)
+    b, db, _k2 = _buffer(dst)
+    if not (da and db):
+        raise TypeError("cardiac_probe takes device tensors")
+    _check(ctx, _lib.cardiac_probe(ctx, what, a, b, n))
 
 
 def cardiac_launch_count(ctx) -> int:

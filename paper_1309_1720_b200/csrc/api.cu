@@ -211,7 +211,8 @@ cardiac_ctx* cardiac_create(int model, int nx, int ny, double dx, double dt, int
     return bad("Rush-Larsen / implicit Euler are defined for the BOCF gates only");
   const int r = stencil_radius(stencil);
   if (nx < 2 * r + 1 || ny < 2 * r + 1) return bad("nx, ny must be >= 2*radius+1");
-  if (nx > (1 << 20) || ny > (1 << 20)) return bad("nx, ny too large");
+  if (nx > (1 << 20) || ny > (1 << 20) || (long long)((nx + 15) / 16 * 16) * ny >= (1LL << 31))
+    return bad("grid too large (a field must have fewer than 2^31 elements)");
   if (batch < 1 || batch > 65535) return bad("batch must be in [1, 65535]");
   if (!(dx > 0.0) || !std::isfinite(dx)) return bad("dx must be finite and > 0");
   if (!(dt > 0.0) || !std::isfinite(dt)) return bad("dt must be finite and > 0");
@@ -390,6 +391,18 @@ int cardiac_get_jvp(cardiac_ctx* c, double eps, double* dst, int dst_on_device) 
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
   cudaFree(tmp);
   if (e != cudaSuccess) return fail_cuda(c, e, "jvp");
+  c->launches++;
+  return CARDIAC_OK;
+}
+
+int cardiac_probe(cardiac_ctx* c, int what, const double* in_dev, double* out_dev, long long n) {
+  if (!c) return CARDIAC_ERR_INVALID;
+  if (!in_dev || !out_dev || n < 0) return fail(c, CARDIAC_ERR_INVALID, "bad probe arguments");
+  if (what < CARDIAC_PROBE_EXP || what > CARDIAC_PROBE_REACTION)
+    return fail(c, CARDIAC_ERR_INVALID, "unknown probe");
+  DeviceGuard guard(c->device);
+  cudaError_t e = launch_probe(c->pb, what, in_dev, out_dev, n, c->stream);
+  if (e != cudaSuccess) return fail_cuda(c, e, "probe launch");
   c->launches++;
   return CARDIAC_OK;
 }

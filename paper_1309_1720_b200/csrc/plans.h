@@ -33,4 +33,9 @@ cudaError_t launch_stage(const Problem& pb, const StageLaunch& st, cudaStream_t 
 cudaError_t launch_jvp(const Problem& pb, const double* state, double eps, double* dst_dense,
                        cudaStream_t stream);
 
+// probe_kernels.cu: diagnostic evaluation of the device math / reactions on sample points
+enum { PROBE_EXP = 0, PROBE_RCP = 1, PROBE_HK = 2, PROBE_REACTION = 3 };
+cudaError_t launch_probe(const Problem& pb, int what, const double* in, double* out, long long n,
+                         cudaStream_t stream);
+
 }  // namespace cardiac

@@ -6,6 +6,12 @@
 // kernel: each thread evaluates the stencil of every diffusing field, the pointwise reaction with
 // the gating variables in registers, and the RK combination, and stores the next stage value.
 // The kernel boundary is the paper's "lock-step" synchronisation.
+//
+// Layout of the work: a thread owns TWO x-adjacent cells (one 128-bit load/store per field, the
+// paper's "vector width 2 for doubles"); a 32x8 block owns a 64x8 tile.  Blocks whose
+// tile plus stencil halo lies inside the grid take a branch-free path with 128-bit neighbour loads
+// served by L1; only the blocks on the rim pay for the index reflection of the no-flux boundary
+// ("branching threads incur some performance penalty").
 #include "plans.h"
 #include "stage.cuh"
 
@@ -13,55 +19,69 @@ namespace cardiac {
 
 namespace {
 
-constexpr int TX = 32, TY = 8;
+constexpr int TX = 32, TY = 8;   // threads; the tile is 2*TX x TY cells
 
-template <class MD, int STENCIL, int KIND>
-__global__ void __launch_bounds__(TX* TY)
-    stage_direct_kernel(const __grid_constant__ StageArgs<MD> a) {
-  constexpr int NV = MD::NV, ND = MD::ND;
-  const int i = blockIdx.x * TX + threadIdx.x;
-  const int j = blockIdx.y * TY + threadIdx.y;
-  const int nx = a.g.nx, ny = a.g.ny, bc = a.g.boundary;
-  if (i >= nx || j >= ny) return;
-  const long long base = (long long)blockIdx.z * a.g.bstride;
-  const long long row = (long long)j * a.g.pitch;
-  const long long c = base + row + i;
-  const double* __restrict__ in = a.in;
+CARDIAC_D double2 ld2(const double* p) { return *reinterpret_cast<const double2*>(p); }
+CARDIAC_D void st2(double* p, double a, double b) { *reinterpret_cast<double2*>(p) = make_double2(a, b); }
 
-  double z[NV], f[NV];
-#pragma unroll
-  for (int q = 0; q < NV; ++q) z[q] = in[c + q * a.g.fstride];
-  MD::reaction(a.p, z, f);
-
-  // neighbour offsets with the boundary rule applied per axis (Q3)
-  const long long rw1 = bidx(i - 1, nx, bc), re1 = bidx(i + 1, nx, bc);
-  const long long rs1 = (long long)bidx(j - 1, ny, bc) * a.g.pitch;
-  const long long rn1 = (long long)bidx(j + 1, ny, bc) * a.g.pitch;
-#pragma unroll
-  for (int q = 0; q < ND; ++q) {
-    const double* __restrict__ U = in + base + q * a.g.fstride;
-    double s;
-    if (STENCIL == S_LAP5) {
-      s = Stencil<S_LAP5>::apply(z[q], U[row + rw1], U[row + re1], U[rs1 + i], U[rn1 + i]);
-    } else if (STENCIL == S_LAP9X4) {
-      const long long rw2 = bidx(i - 2, nx, bc), re2 = bidx(i + 2, nx, bc);
-      const long long rs2 = (long long)bidx(j - 2, ny, bc) * a.g.pitch;
-      const long long rn2 = (long long)bidx(j + 2, ny, bc) * a.g.pitch;
-      s = Stencil<S_LAP9X4>::apply(z[q], U[row + rw1], U[row + re1], U[rs1 + i], U[rn1 + i],
-                                   U[row + rw2], U[row + re2], U[rs2 + i], U[rn2 + i]);
-    } else {
-      s = Stencil<S_BOX9>::apply(z[q], U[row + rw1], U[row + re1], U[rs1 + i], U[rn1 + i],
-                                 U[rs1 + rw1], U[rs1 + re1], U[rn1 + rw1], U[rn1 + re1]);
-    }
-    f[q] = fma(a.lapw[q], s, f[q]);
+// integer-weight stencil sums of the two cells (x, x+1) of row `row`; interior, no boundary logic
+template <int STENCIL>
+CARDIAC_D void stencil_pair(const double* __restrict__ U, int row, int x, int pitch, double2 c,
+                            double& s0, double& s1) {
+  const double* p = U + row + x;
+  if (STENCIL == S_LAP5) {
+    const double w = p[-1], e = p[2];
+    const double2 s = ld2(p - pitch), n = ld2(p + pitch);
+    s0 = Stencil<S_LAP5>::apply(c.x, w, c.y, s.x, n.x);
+    s1 = Stencil<S_LAP5>::apply(c.y, c.x, e, s.y, n.y);
+  } else if (STENCIL == S_LAP9X4) {
+    const double2 l = ld2(p - 2), r = ld2(p + 2);
+    const double2 a1 = ld2(p - pitch), b1 = ld2(p + pitch);
+    const double2 a2 = ld2(p - 2 * pitch), b2 = ld2(p + 2 * pitch);
+    s0 = Stencil<S_LAP9X4>::apply(c.x, l.y, c.y, a1.x, b1.x, l.x, r.x, a2.x, b2.x);
+    s1 = Stencil<S_LAP9X4>::apply(c.y, c.x, r.x, a1.y, b1.y, l.y, r.y, a2.y, b2.y);
+  } else {
+    const double w = p[-1], e = p[2];
+    const double2 s = ld2(p - pitch), n = ld2(p + pitch);
+    const double sw = p[-pitch - 1], se = p[-pitch + 2], nw = p[pitch - 1], ne = p[pitch + 2];
+    s0 = Stencil<S_BOX9>::apply(c.x, w, c.y, s.x, n.x, sw, s.y, nw, n.y);
+    s1 = Stencil<S_BOX9>::apply(c.y, c.x, e, s.y, n.y, s.x, se, n.x, ne);
   }
+}
 
+// one cell with the boundary rule applied per axis (Q3)
+template <int STENCIL>
+CARDIAC_D double stencil_edge(const double* __restrict__ U, int i, int j, int nx, int ny, int pitch,
+                              int bc, double c) {
+  const int rw1 = bidx(i - 1, nx, bc), re1 = bidx(i + 1, nx, bc);
+  const int row = j * pitch;
+  const int rs1 = bidx(j - 1, ny, bc) * pitch, rn1 = bidx(j + 1, ny, bc) * pitch;
+  if (STENCIL == S_LAP5) {
+    return Stencil<S_LAP5>::apply(c, U[row + rw1], U[row + re1], U[rs1 + i], U[rn1 + i]);
+  } else if (STENCIL == S_LAP9X4) {
+    const int rw2 = bidx(i - 2, nx, bc), re2 = bidx(i + 2, nx, bc);
+    const int rs2 = bidx(j - 2, ny, bc) * pitch, rn2 = bidx(j + 2, ny, bc) * pitch;
+    return Stencil<S_LAP9X4>::apply(c, U[row + rw1], U[row + re1], U[rs1 + i], U[rn1 + i],
+                                    U[row + rw2], U[row + re2], U[rs2 + i], U[rn2 + i]);
+  } else {
+    return Stencil<S_BOX9>::apply(c, U[row + rw1], U[row + re1], U[rs1 + i], U[rn1 + i],
+                                  U[rs1 + rw1], U[rs1 + re1], U[rn1 + rw1], U[rn1 + re1]);
+  }
+}
+
+// the update of one cell once f = D lap + N is known; o = offset of the cell inside its field
+template <class MD, int KIND>
+CARDIAC_D void finish_cell(const StageArgs<MD>& a, const double* __restrict__ yb,
+                           const double* __restrict__ Ab, const double* __restrict__ Bb,
+                           double* __restrict__ ob, int o, const double (&z)[MD::NV],
+                           const double (&f)[MD::NV]) {
+  constexpr int NV = MD::NV;
   if (KIND == K_RL || KIND == K_IE) {
     // BOCF only: u explicit Euler; gates with coefficients frozen at u^n
-    if constexpr (MD::NV == 4) {
+    if constexpr (NV == 4) {
       double alpha[3], beta[3];
       MD::gates(a.p, z[0], alpha, beta);
-      a.out[c] = fma(a.dt, f[0], z[0]);
+      ob[o] = fma(a.dt, f[0], z[0]);
 #pragma unroll
       for (int g = 0; g < 3; ++g) {
         double x = z[g + 1], xn;
@@ -72,34 +92,111 @@ __global__ void __launch_bounds__(TX* TY)
         } else {
           xn = fma(a.dt, beta[g], x) / fma(-a.dt, alpha[g], 1.0);
         }
-        a.out[c + (g + 1) * a.g.fstride] = xn;
+        ob[o + (g + 1) * a.g.fstride] = xn;
       }
     }
     return;
   }
-
 #pragma unroll
   for (int q = 0; q < NV; ++q) {
-    const long long cq = c + q * a.g.fstride;
+    const long long oq = o + q * a.g.fstride;
     double yv = 0.0, Av = 0.0, Bv = 0.0;
-    if (KIND != K_SELF) yv = a.y[cq];
-    if (KIND == K_RK4F) { Av = a.A[cq]; Bv = a.B[cq]; }
-    a.out[cq] = combine<KIND>(a.w_y, a.w_in, a.w_A, a.w_B, a.w_f, yv, z[q], Av, Bv, f[q]);
+    if (KIND != K_SELF) yv = yb[oq];
+    if (KIND == K_RK4F) { Av = Ab[oq]; Bv = Bb[oq]; }
+    ob[oq] = combine<KIND>(a.w_y, a.w_in, a.w_A, a.w_B, a.w_f, yv, z[q], Av, Bv, f[q]);
+  }
+}
+
+template <class MD, int STENCIL, int KIND>
+__global__ void __launch_bounds__(TX* TY)
+    stage_kernel(const __grid_constant__ StageArgs<MD> a) {
+  constexpr int NV = MD::NV, ND = MD::ND;
+  constexpr int R = stencil_radius(STENCIL);
+  const int nx = a.g.nx, ny = a.g.ny, pitch = a.g.pitch;
+  const int x0 = blockIdx.x * (2 * TX), j0 = blockIdx.y * TY;
+  const int x = x0 + 2 * threadIdx.x, j = j0 + threadIdx.y;
+  const long long base = (long long)blockIdx.z * a.g.bstride;
+  const double* __restrict__ in = a.in + base;
+  const double* __restrict__ yb = a.y + base;
+  const double* __restrict__ Ab = a.A + base;
+  const double* __restrict__ Bb = a.B + base;
+  double* __restrict__ ob = a.out + base;
+
+  // block-uniform: tile and halo inside the grid -> no boundary logic, 128-bit accesses
+  const bool interior = x0 >= 2 && x0 + 2 * TX + 2 <= nx && j0 >= R && j0 + TY + R <= ny;
+  if (interior && KIND != K_RL && KIND != K_IE) {
+    const int row = j * pitch, o = row + x;
+    double2 zz[NV];
+#pragma unroll
+    for (int q = 0; q < NV; ++q) zz[q] = ld2(in + o + q * a.g.fstride);
+    double2 yy[NV] = {}, AA[NV] = {}, BB[NV] = {};
+    if (KIND != K_SELF) {
+#pragma unroll
+      for (int q = 0; q < NV; ++q) yy[q] = ld2(yb + o + q * a.g.fstride);
+    }
+    if (KIND == K_RK4F) {
+#pragma unroll
+      for (int q = 0; q < NV; ++q) {
+        AA[q] = ld2(Ab + o + q * a.g.fstride);
+        BB[q] = ld2(Bb + o + q * a.g.fstride);
+      }
+    }
+    double z0[NV], z1[NV], f0[NV], f1[NV];
+#pragma unroll
+    for (int q = 0; q < NV; ++q) { z0[q] = zz[q].x; z1[q] = zz[q].y; }
+    MD::reaction(a.p, z0, f0);
+    MD::reaction(a.p, z1, f1);
+#pragma unroll
+    for (int q = 0; q < ND; ++q) {
+      double s0, s1;
+      stencil_pair<STENCIL>(in + q * a.g.fstride, row, x, pitch, zz[q], s0, s1);
+      f0[q] = fma(a.lapw[q], s0, f0[q]);
+      f1[q] = fma(a.lapw[q], s1, f1[q]);
+    }
+#pragma unroll
+    for (int q = 0; q < NV; ++q) {
+      double r0 = combine<KIND>(a.w_y, a.w_in, a.w_A, a.w_B, a.w_f, yy[q].x, z0[q], AA[q].x, BB[q].x, f0[q]);
+      double r1 = combine<KIND>(a.w_y, a.w_in, a.w_A, a.w_B, a.w_f, yy[q].y, z1[q], AA[q].y, BB[q].y, f1[q]);
+      st2(ob + o + q * a.g.fstride, r0, r1);
+    }
+    return;
+  }
+
+  // rim blocks (and the gate integrators): one cell at a time, boundary rule per neighbour
+  if (j >= ny) return;
+  const int bc = a.g.boundary;
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    const int i = x + h;
+    if (i >= nx) break;
+    const int o = j * pitch + i;
+    double z[NV], f[NV];
+#pragma unroll
+    for (int q = 0; q < NV; ++q) z[q] = in[o + q * a.g.fstride];
+    MD::reaction(a.p, z, f);
+#pragma unroll
+    for (int q = 0; q < ND; ++q) {
+      double s = stencil_edge<STENCIL>(in + q * a.g.fstride, i, j, nx, ny, pitch, bc, z[q]);
+      f[q] = fma(a.lapw[q], s, f[q]);
+    }
+    finish_cell<MD, KIND>(a, yb, Ab, Bb, ob, o, z, f);
   }
 }
 
 template <class MD, int STENCIL, int KIND>
 cudaError_t run(const Problem& pb, const StageLaunch& st, cudaStream_t stream) {
   StageArgs<MD> a;
-  a.in = st.in; a.y = st.y; a.A = st.A; a.B = st.B; a.out = st.out;
+  // unused operands alias the input so that every pointer the kernel forms is valid
+  a.in = st.in; a.y = st.y ? st.y : st.in; a.A = st.A ? st.A : st.in; a.B = st.B ? st.B : st.in;
+  a.out = st.out;
   a.g.nx = pb.nx; a.g.ny = pb.ny; a.g.pitch = pb.pitch; a.g.boundary = pb.boundary;
   a.g.fstride = pb.fstride; a.g.bstride = pb.bstride;
   a.w_y = st.w_y; a.w_in = st.w_in; a.w_A = st.w_A; a.w_B = st.w_B; a.w_f = st.w_f;
   a.dt = pb.dt;
   MD::derive(pb.params, a.p);
   for (int q = 0; q < MD::ND; ++q) a.lapw[q] = a.p.D[q] * stencil_norm(STENCIL) / (pb.dx * pb.dx);
-  dim3 grid((pb.nx + TX - 1) / TX, (pb.ny + TY - 1) / TY, pb.batch), block(TX, TY);
-  stage_direct_kernel<MD, STENCIL, KIND><<<grid, block, 0, stream>>>(a);
+  dim3 grid((pb.nx + 2 * TX - 1) / (2 * TX), (pb.ny + TY - 1) / TY, pb.batch), block(TX, TY);
+  stage_kernel<MD, STENCIL, KIND><<<grid, block, 0, stream>>>(a);
   return cudaGetLastError();
 }
 
@@ -131,7 +228,7 @@ cudaError_t by_stencil(const Problem& pb, const StageLaunch& st, cudaStream_t s)
 
 __global__ void jvp_kernel(const double* __restrict__ Z, double* __restrict__ J, int nx, int ny,
                            int nv, int pitch, long long bstride, double eps) {
-  // one thread per output element of member blockIdx.z + 1
+  // one thread per output element of member blockIdx.y + 1
   const long long n = (long long)nx * ny * nv;
   const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= n) return;

@@ -74,8 +74,34 @@ void carve(cardiac_ctx* c) {
   for (int b = 0; b < c->nbuf; ++b) c->buf[b] = (double*)c->ws + b * n;
 }
 
+// AUTO: the on-chip tile engine wherever a time step is cheap enough per cell that the global
+// round trip per substep dominates (FHN, Karma); the 4-field ionic model is FP64-pipe bound and its
+// register-resident patches are too small to amortise an 8-cell halo, so it stays stage-synchronous
+// (DESIGN.md "Plans").
+int auto_plan(const Problem& pb) {
+  const bool rk_like = pb.integrator == I_EULER || pb.integrator == I_HEUN || pb.integrator == I_RK4;
+  if (rk_like && pb.model != CARDIAC_BOCF) return CARDIAC_PLAN_FUSED;
+  return CARDIAC_PLAN_STAGE;
+}
+
+// Plan FUSED: one launch advances `ksteps` time steps (1, or kEulerBlock Euler steps), ping-pong.
+int enqueue_fused(cardiac_ctx* c, cudaStream_t s, int ksteps) {
+  TileLaunch tl{c->buf[c->cur], c->buf[1 - c->cur], ksteps};
+  cudaError_t e = launch_fused(c->pb, tl, s);
+  if (e != cudaSuccess) return fail_cuda(c, e, "fused launch");
+  c->launches++;
+  c->cur ^= 1;
+  return CARDIAC_OK;
+}
+
+// time steps advanced by one repetition unit of the plan
+int unit_steps(const cardiac_ctx* c) {
+  return (c->plan == CARDIAC_PLAN_FUSED && c->pb.integrator == I_EULER) ? c->plan_param : 1;
+}
+
 // Enqueue the kernels of ONE time step on `s`; advances c->cur as the real execution would.
 int enqueue_step(cardiac_ctx* c, cudaStream_t s) {
+  if (c->plan == CARDIAC_PLAN_FUSED) return enqueue_fused(c, s, 1);
   const Problem& pb = c->pb;
   const double dt = pb.dt;
   StageLaunch st{};
@@ -89,13 +115,18 @@ int enqueue_step(cardiac_ctx* c, cudaStream_t s) {
     return CARDIAC_OK;
   };
   int rc = CARDIAC_OK;
-  double** b = c->buf;
+  // b[0] holds the state; b[1..] are the other buffers (the state may sit in buffer 1 after an
+  // odd number of ping-pong launches)
+  double* b[kMaxBuf];
+  b[0] = c->buf[c->cur];
+  for (int i = 0, n = 1; i < c->nbuf; ++i)
+    if (i != c->cur) b[n++] = c->buf[i];
   switch (pb.integrator) {
     case I_EULER:
     case I_RUSH_LARSEN:
     case I_IMPLICIT_EULER: {
       int kind = pb.integrator == I_EULER ? K_SELF : (pb.integrator == I_RUSH_LARSEN ? K_RL : K_IE);
-      rc = go(kind, b[c->cur], nullptr, nullptr, nullptr, b[1 - c->cur], 0, 0, 0, 0, dt);
+      rc = go(kind, b[0], nullptr, nullptr, nullptr, b[1], 0, 0, 0, 0, dt);
       c->cur ^= 1;
       break;
     }
@@ -119,13 +150,15 @@ int enqueue_step(cardiac_ctx* c, cudaStream_t s) {
   return rc;
 }
 
-// Capture `steps` time steps starting from parity `cur` into an executable graph.
-int build_graph(cardiac_ctx* c, int steps) {
+// Capture `units` repetition units starting from parity `cur` into an executable graph.
+int build_graph(cardiac_ctx* c, int units) {
   int parity = c->cur;
   long long launches_before = c->launches;
   CK(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
   int rc = CARDIAC_OK;
-  for (int s = 0; s < steps && rc == CARDIAC_OK; ++s) rc = enqueue_step(c, c->cap_stream);
+  const int us = unit_steps(c);
+  for (int s = 0; s < units && rc == CARDIAC_OK; ++s)
+    rc = us == 1 ? enqueue_step(c, c->cap_stream) : enqueue_fused(c, c->cap_stream, us);
   cudaGraph_t g = nullptr;
   cudaError_t e = cudaStreamEndCapture(c->cap_stream, &g);
   c->cur = parity;  // capture executed nothing
@@ -135,7 +168,7 @@ int build_graph(cardiac_ctx* c, int steps) {
   e = cudaGraphInstantiate(&c->graph[parity], g, 0);
   cudaGraphDestroy(g);
   if (e != cudaSuccess) return fail_cuda(c, e, "cudaGraphInstantiate");
-  c->graph_steps = steps;
+  c->graph_steps = units;
   return CARDIAC_OK;
 }
 
@@ -242,6 +275,9 @@ cardiac_ctx* cardiac_create(int model, int nx, int ny, double dx, double dt, int
   cardiac_default_params(model, pb.params, c->nparams);
   c->device = dev;
   c->nbuf = buffers_of(integ);
+  c->plan_req = CARDIAC_PLAN_AUTO;
+  c->plan = auto_plan(pb);
+  c->plan_param = (c->plan == CARDIAC_PLAN_FUSED && integ == I_EULER) ? kEulerBlock : 0;
   e = cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking);
   if (e != cudaSuccess) {
     delete c;
@@ -279,12 +315,27 @@ int cardiac_set_stream(cardiac_ctx* c, void* cuda_stream) {
 
 int cardiac_set_plan(cardiac_ctx* c, int plan, int param) {
   if (!c) return CARDIAC_ERR_INVALID;
-  if (plan != CARDIAC_PLAN_AUTO && plan != CARDIAC_PLAN_STAGE)
+  int resolved = plan, rparam = 0;
+  const int integ = c->pb.integrator;
+  const bool rk_like = integ == I_EULER || integ == I_HEUN || integ == I_RK4;
+  if (plan == CARDIAC_PLAN_AUTO) resolved = auto_plan(c->pb);
+  if (resolved == CARDIAC_PLAN_STAGE) {
+    if (param != 0) return fail(c, CARDIAC_ERR_INVALID, "plan parameter must be 0");
+  } else if (resolved == CARDIAC_PLAN_FUSED) {
+    if (!rk_like) return fail(c, CARDIAC_ERR_INVALID, "FUSED supports Euler, Heun and RK4 only");
+    if (integ == I_EULER) {
+      rparam = param == 0 ? kEulerBlock : param;
+      if (rparam != 1 && rparam != kEulerBlock)
+        return fail(c, CARDIAC_ERR_INVALID, "FUSED + Euler: steps per launch must be 1 or 4");
+    } else if (param != 0) {
+      return fail(c, CARDIAC_ERR_INVALID, "plan parameter must be 0");
+    }
+  } else {
     return fail(c, CARDIAC_ERR_INVALID, "plan not available for this context");
-  if (param != 0) return fail(c, CARDIAC_ERR_INVALID, "plan parameter must be 0");
+  }
   c->plan_req = plan;
-  c->plan = CARDIAC_PLAN_STAGE;
-  c->plan_param = param;
+  c->plan = resolved;
+  c->plan_param = rparam;
   drop_graphs(c);
   return CARDIAC_OK;
 }
@@ -346,23 +397,29 @@ int cardiac_step(cardiac_ctx* c, long long nsteps) {
   if (!c->has_state) return fail(c, CARDIAC_ERR_NOSTATE, "no state set");
   if (nsteps == 0) return CARDIAC_OK;
   DeviceGuard guard(c->device);
-  const int ns = stages_of(c->pb.integrator);
-  int gsteps = kGraphNodes / ns;
-  if (gsteps & 1) gsteps++;  // even: ping-pong integrators end on the parity they started on
+  const int us = unit_steps(c);                                        // time steps per unit
+  const int ul = c->plan == CARDIAC_PLAN_FUSED ? 1 : stages_of(c->pb.integrator);  // launches per unit
+  int gunits = kGraphNodes / ul;
+  if (gunits & 1) gunits++;  // even: ping-pong plans end on the parity they started on
+  const long long gsteps = (long long)gunits * us;
   long long left = nsteps;
   if (left >= gsteps) {
-    if (c->graph_steps != gsteps) drop_graphs(c);
+    if (c->graph_steps != gunits) drop_graphs(c);
     if (!c->graph[c->cur]) {
-      int rc = build_graph(c, gsteps);
+      int rc = build_graph(c, gunits);
       if (rc) return rc;
     }
     while (left >= gsteps) {
       CK(cudaGraphLaunch(c->graph[c->cur], c->stream));
-      c->launches += (long long)gsteps * ns;
+      c->launches += (long long)gunits * ul;
       left -= gsteps;
     }
   }
-  for (; left > 0; --left) {
+  for (; left >= us; left -= us) {
+    int rc = us == 1 ? enqueue_step(c, c->stream) : enqueue_fused(c, c->stream, us);
+    if (rc) return rc;
+  }
+  for (; left > 0; --left) {  // fewer Euler steps than one temporal block
     int rc = enqueue_step(c, c->stream);
     if (rc) return rc;
   }

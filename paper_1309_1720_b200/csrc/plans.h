@@ -33,6 +33,23 @@ cudaError_t launch_stage(const Problem& pb, const StageLaunch& st, cudaStream_t 
 cudaError_t launch_jvp(const Problem& pb, const double* state, double eps, double* dst_dense,
                        cudaStream_t stream);
 
+// tile_kernels_*.cu: plan FUSED — all substeps of one time step (ksteps = 1), or ksteps forward-Euler
+// steps, in one launch on overlapped tiles (tile.cuh).  in != out.
+constexpr int kEulerBlock = 4;  // Euler steps per launch when temporally blocked
+struct TileLaunch {
+  const double* in;
+  double* out;
+  int ksteps;
+};
+cudaError_t launch_fused_fhn(const Problem& pb, const TileLaunch& tl, cudaStream_t stream);
+cudaError_t launch_fused_karma(const Problem& pb, const TileLaunch& tl, cudaStream_t stream);
+cudaError_t launch_fused_bocf(const Problem& pb, const TileLaunch& tl, cudaStream_t stream);
+inline cudaError_t launch_fused(const Problem& pb, const TileLaunch& tl, cudaStream_t stream) {
+  return pb.model == 0 ? launch_fused_fhn(pb, tl, stream)
+                       : (pb.model == 1 ? launch_fused_karma(pb, tl, stream)
+                                        : launch_fused_bocf(pb, tl, stream));
+}
+
 // probe_kernels.cu: diagnostic evaluation of the device math / reactions on sample points
 enum { PROBE_EXP = 0, PROBE_RCP = 1, PROBE_HK = 2, PROBE_REACTION = 3 };
 cudaError_t launch_probe(const Problem& pb, int what, const double* in, double* out, long long n,

@@ -1,0 +1,94 @@
+// tile_dispatch.cuh — kernels and host dispatch of plan FUSED for one model; included by the
+// per-model tile_kernels_*.cu files so that the (large, fully unrolled) instantiations compile in
+// parallel.
+#pragma once
+#include "plans.h"
+#include "tile.cuh"
+
+namespace cardiac {
+
+// window geometry per (model, halo): 2*NTX x PR*NTY cells, NTX*NTY threads, one CTA per SM.
+// The 4-field ionic model keeps 11 doubles per cell in registers, so its patches are smaller.
+template <class MD, int H>
+struct FusedGeom {
+  using type = TileGeom<40, 12, 4>;  // 80 x 48 window, 480 threads
+};
+template <int VARIANT, int H>
+struct FusedGeom<Model<M_BOCF, VARIANT>, H> {
+  using type = TileGeom<24, 16, 2>;  // 48 x 32 window, 384 threads
+};
+
+template <class MD, int STENCIL, int INTEG, int KSTEPS, class TG>
+__global__ void __launch_bounds__(TG::NT, 1)
+    fused_step_kernel(const __grid_constant__ TileArgs<MD> a) {
+  using E = TileEngine<MD, STENCIL, INTEG, KSTEPS, TG>;
+  extern __shared__ double2 smem_fused[];
+  const long long base = (long long)blockIdx.z * a.g.bstride;
+  E::run(a, a.in + base, a.out + base, blockIdx.x, blockIdx.y, reinterpret_cast<double*>(smem_fused));
+}
+
+template <class MD>
+void fill_tile_args(const Problem& pb, int stencil, TileArgs<MD>& a) {
+  a.g.nx = pb.nx; a.g.ny = pb.ny; a.g.pitch = pb.pitch; a.g.boundary = pb.boundary;
+  a.g.fstride = pb.fstride; a.g.bstride = pb.bstride;
+  const double dt = pb.dt;
+  for (int s = 0; s < 4; ++s) a.a_dt[s] = a.b_dt[s] = 0.0;
+  if (pb.integrator == I_RK4) {
+    // Y2 = y + dt/2 k1, Y3 = y + dt/2 k2, Y4 = y + dt k3; y+ = y + dt/6 (k1 + 2 k2 + 2 k3 + k4)
+    a.a_dt[0] = 0.5 * dt; a.a_dt[1] = 0.5 * dt; a.a_dt[2] = dt;
+    a.b_dt[0] = dt / 6.0; a.b_dt[1] = dt / 3.0; a.b_dt[2] = dt / 3.0; a.b_dt[3] = dt / 6.0;
+  } else if (pb.integrator == I_HEUN) {
+    a.a_dt[0] = dt; a.b_dt[0] = 0.5 * dt; a.b_dt[1] = 0.5 * dt;
+  } else {
+    a.a_dt[0] = dt;
+  }
+  MD::derive(pb.params, a.p);
+  for (int q = 0; q < MD::ND; ++q) a.lapw[q] = a.p.D[q] * stencil_norm(stencil) / (pb.dx * pb.dx);
+  a.bufA = a.bufB = nullptr; a.flags = nullptr; a.abort_flag = nullptr;
+  a.nsteps = 0; a.tiles_x = a.tiles_y = 0; a.step_base = 0;
+}
+
+template <class MD, int STENCIL, int INTEG, int KSTEPS>
+cudaError_t fused_run(const Problem& pb, const TileLaunch& tl, cudaStream_t stream) {
+  constexpr int H = stencil_radius(STENCIL) * StepScheme<INTEG, KSTEPS>::NS;
+  using TG = typename FusedGeom<MD, H>::type;
+  using E = TileEngine<MD, STENCIL, INTEG, KSTEPS, TG>;
+  auto kern = fused_step_kernel<MD, STENCIL, INTEG, KSTEPS, TG>;
+  static bool configured = false;  // per instantiation
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, E::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  TileArgs<MD> a;
+  fill_tile_args<MD>(pb, STENCIL, a);
+  a.in = tl.in; a.out = tl.out;
+  dim3 grid((pb.nx + E::TW - 1) / E::TW, (pb.ny + E::TH - 1) / E::TH, pb.batch);
+  kern<<<grid, TG::NT, E::SMEM_BYTES, stream>>>(a);
+  return cudaGetLastError();
+}
+
+template <class MD, int STENCIL>
+cudaError_t fused_by_integrator(const Problem& pb, const TileLaunch& tl, cudaStream_t s) {
+  switch (pb.integrator) {
+    case I_RK4: return fused_run<MD, STENCIL, I_RK4, 1>(pb, tl, s);
+    case I_HEUN: return fused_run<MD, STENCIL, I_HEUN, 1>(pb, tl, s);
+    case I_EULER:
+      if (tl.ksteps == 1) return fused_run<MD, STENCIL, I_EULER, 1>(pb, tl, s);
+      if (tl.ksteps == kEulerBlock) return fused_run<MD, STENCIL, I_EULER, kEulerBlock>(pb, tl, s);
+      break;
+  }
+  return cudaErrorInvalidValue;
+}
+
+template <class MD>
+cudaError_t fused_by_stencil(const Problem& pb, const TileLaunch& tl, cudaStream_t s) {
+  switch (pb.stencil) {
+    case S_LAP5: return fused_by_integrator<MD, S_LAP5>(pb, tl, s);
+    case S_LAP9X4: return fused_by_integrator<MD, S_LAP9X4>(pb, tl, s);
+    case S_BOX9: return fused_by_integrator<MD, S_BOX9>(pb, tl, s);
+  }
+  return cudaErrorInvalidValue;
+}
+
+}  // namespace cardiac

@@ -52,14 +52,19 @@ CASES = [(m, s, i) for m in (FHN, KARMA, BOCF) for s in (LAP5, LAP9X4, BOX9) for
 CASES += [(BOCF, s, i) for s in (LAP5, LAP9X4, BOX9) for i in (RL, IE)]
 
 
-@pytest.mark.parametrize("model,stencil,integ", CASES)
-def test_parity_one_and_hundred_steps(C, model, stencil, integ):
-    # 70 x 45: several 32x8 / 64-wide tiles and a ragged tail in both directions, odd pitch padding
+STAGE, FUSED = 1, 2      # CARDIAC_PLAN_*
+PLAN_CASES = [(m, s, i, STAGE) for (m, s, i) in CASES] + [(m, s, i, FUSED) for (m, s, i) in CASES if i in (EULER, HEUN, RK4)]
+
+
+@pytest.mark.parametrize("model,stencil,integ,plan", PLAN_CASES)
+def test_parity_one_and_hundred_steps(C, model, stencil, integ, plan):
+    # 70 x 45: several 64x8 stage tiles / 2x2 fused tiles and a ragged tail in both directions,
+    # odd width (scalar tail of the 128-bit path), pitch padding
     cfg, Z = make(model, 70, 45, stencil, integ)
-    got1 = gpu_run(C, cfg, Z, 1)
+    got1 = gpu_run(C, cfg, Z, 1, plan=plan)
     ref1 = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 1)
     assert maxabs(got1, ref1) <= TOL_1
-    got = gpu_run(C, cfg, Z, 100)
+    got = gpu_run(C, cfg, Z, 100, plan=plan)
     ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 100)
     assert np.all(np.isfinite(got))
     assert maxabs(got, ref) <= TOL_100
@@ -68,17 +73,19 @@ def test_parity_one_and_hundred_steps(C, model, stencil, integ):
 
 @pytest.mark.parametrize("model,stencil,integ", [(FHN, LAP9X4, RK4), (KARMA, LAP5, RK4), (BOCF, LAP9X4, RK4),
                                                  (FHN, LAP5, EULER), (BOCF, BOX9, HEUN)])
-def test_parity_periodic_boundary(C, model, stencil, integ):
+@pytest.mark.parametrize("plan", [STAGE, FUSED])
+def test_parity_periodic_boundary(C, model, stencil, integ, plan):
     cfg, Z = make(model, 37, 50, stencil, integ, boundary=1)
-    got = gpu_run(C, cfg, Z, 30)
+    got = gpu_run(C, cfg, Z, 30, plan=plan)
     ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 30)
     assert maxabs(got, ref) <= TOL_100
 
 
 @pytest.mark.parametrize("model", [KARMA, BOCF])
-def test_parity_tanhfree_variant(C, model):
+@pytest.mark.parametrize("plan", [STAGE, FUSED])
+def test_parity_tanhfree_variant(C, model, plan):
     cfg, Z = make(model, 40, 33, LAP9X4, RK4, variant=1)
-    got = gpu_run(C, cfg, Z, 50)
+    got = gpu_run(C, cfg, Z, 50, plan=plan)
     ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 50)
     assert maxabs(got, ref) <= TOL_100
     ref_paper = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme & 0xFFFFFF, 50)
@@ -87,36 +94,68 @@ def test_parity_tanhfree_variant(C, model):
 
 @pytest.mark.parametrize("model,stencil,nx,ny", [(FHN, LAP5, 3, 3), (FHN, LAP9X4, 5, 5), (KARMA, LAP9X4, 5, 64),
                                                  (BOCF, LAP5, 200, 3), (FHN, BOX9, 3, 17), (KARMA, LAP5, 33, 4)])
-def test_parity_degenerate_sizes(C, model, stencil, nx, ny):
-    """Minimum sizes 2r+1 (every stencil arm reflects) and thin strips."""
+@pytest.mark.parametrize("plan", [STAGE, FUSED])
+def test_parity_degenerate_sizes(C, model, stencil, nx, ny, plan):
+    """Minimum sizes 2r+1 (every stencil arm reflects; the fused window folds the grid several
+    times over) and thin strips."""
     cfg, Z = make(model, nx, ny, stencil, RK4)
-    got = gpu_run(C, cfg, Z, 20)
+    got = gpu_run(C, cfg, Z, 20, plan=plan)
     ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 20)
     assert maxabs(got, ref) <= TOL_100
 
 
-def test_batch_members_independent_of_position(C):
+@pytest.mark.parametrize("plan", [STAGE, FUSED])
+def test_batch_members_independent_of_position(C, plan):
     cfg, Z = make(KARMA, 48, 40, LAP5, RK4, batch=5, seed=3)
-    got = gpu_run(C, cfg, Z, 10)
+    def gpu_run_p(C, cfg, Z, n):
+        return gpu_run(C, cfg, Z, n, plan=plan)
+    got = gpu_run_p(C, cfg, Z, 10)
     ref = O.step(KARMA, Z, cfg.dx, cfg.dt, cfg.scheme, 10)
     assert maxabs(got, ref) <= TOL_100
     perm = [3, 0, 4, 2, 1]
-    got_p = gpu_run(C, cfg, Z[perm], 10)
+    got_p = gpu_run_p(C, cfg, Z[perm], 10)
     assert np.array_equal(got_p, got[perm])                 # bitwise, whatever the slot
     import dataclasses
-    single = gpu_run(C, dataclasses.replace(cfg, batch=1), Z[2:3], 10)
+    single = gpu_run_p(C, dataclasses.replace(cfg, batch=1), Z[2:3], 10)
     assert np.array_equal(single[0], got[2])
 
 
-@pytest.mark.parametrize("model,integ", [(FHN, EULER), (FHN, RK4), (KARMA, HEUN), (BOCF, RL)])
-def test_step_composition_and_determinism_bitwise(C, model, integ):
-    """step(a); step(b) == step(a+b), graph replay == direct launches, run-to-run identical."""
-    cfg, Z = make(model, 64, 37, LAP9X4, integ)
-    whole = gpu_run(C, cfg, Z, 137)                         # graph chunks + remainder
-    parts = gpu_run(C, cfg, Z, 137, chunks=[1, 70, 3, 63])
-    singles = gpu_run(C, cfg, Z, 137, chunks=[1] * 137)    # never reaches a graph
-    again = gpu_run(C, cfg, Z, 137)
+@pytest.mark.parametrize("model,integ,plan", [(FHN, EULER, STAGE), (FHN, RK4, STAGE), (KARMA, HEUN, STAGE),
+                                              (BOCF, RL, STAGE), (FHN, EULER, FUSED), (FHN, RK4, FUSED),
+                                              (KARMA, HEUN, FUSED), (BOCF, EULER, FUSED)])
+def test_step_composition_and_determinism_bitwise(C, model, integ, plan):
+    """step(a); step(b) == step(a+b), graph replay == direct launches, temporally blocked Euler ==
+    single Euler steps, run-to-run identical."""
+    cfg, Z = make(model, 96, 37, LAP9X4, integ)
+    whole = gpu_run(C, cfg, Z, 301, plan=plan)                        # graph chunks + remainder
+    parts = gpu_run(C, cfg, Z, 301, plan=plan, chunks=[1, 70, 3, 227])
+    singles = gpu_run(C, cfg, Z, 301, plan=plan, chunks=[1] * 301)    # never reaches a graph
+    again = gpu_run(C, cfg, Z, 301, plan=plan)
     assert np.array_equal(whole, parts) and np.array_equal(whole, singles) and np.array_equal(whole, again)
+
+
+def test_fused_many_tiles_matches_stage_plan_and_oracle(C):
+    """A grid of 4 x 6 fused tiles with ragged edges: every output cell is written exactly once and
+    halo recomputation agrees with the neighbour's own result."""
+    for model, stencil, integ in [(FHN, LAP9X4, RK4), (KARMA, LAP5, RK4), (FHN, LAP5, EULER), (KARMA, BOX9, HEUN)]:
+        cfg, Z = make(model, 250, 170, stencil, integ, seed=21)
+        got = gpu_run(C, cfg, Z, 12, plan=FUSED)
+        ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 12)
+        assert maxabs(got, ref) <= TOL_100
+        assert maxabs(got, gpu_run(C, cfg, Z, 12, plan=STAGE)) <= 1e-12
+
+
+def test_plan_switch_keeps_state(C):
+    cfg, Z = make(FHN, 70, 45, LAP9X4, RK4)
+    with C.Context.from_config(cfg, plan=FUSED) as ctx:
+        ctx.set_state(Z)
+        ctx.step(3)                                   # odd number of ping-pong launches
+        C.cardiac_set_plan(ctx.ctx, STAGE, 0)
+        ctx.step(4)
+        C.cardiac_set_plan(ctx.ctx, FUSED, 0)
+        ctx.step(2)
+        got = ctx.get_state()
+    assert maxabs(got, O.step(FHN, Z, cfg.dx, cfg.dt, cfg.scheme, 9)) <= TOL_100
 
 
 def test_uniform_state_and_rest_state(C):
@@ -160,6 +199,7 @@ def test_error_paths_and_device_buffers(C):
     cfg, Z = make(FHN, 40, 30, LAP5, EULER)
     ctx = C.cardiac_create(cfg.model, cfg.nx, cfg.ny, cfg.dx, cfg.dt, cfg.scheme, 1)
     try:
+        C.cardiac_set_plan(ctx, STAGE, 0)        # one launch per Euler step: launch counts below
         with pytest.raises(C.CardiacError) as ei:
             C.cardiac_step(ctx, 1)
         assert ei.value.code == C.CARDIAC_ERR_NOSTATE

@@ -54,13 +54,17 @@ def measured_peaks() -> tuple[float, str]:
 
 
 def recorded_traffic(cfg, plan_name):
-    """ncu dram bytes per launch of the dominant kernel, if a capture was committed for this config."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    """ncu dram bytes per launch of the dominant kernel, if a capture was committed for this config
+    (profiles/traffic.csv, written by hand from the .ncu-rep named there)."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(p):
-        try:
-            return json.load(open(p)).get(f"{cfg.name}:{plan_name}")
-        except Exception:
-            return None
+        import csv
+        for row in csv.DictReader(open(p)):
+            if row.get("config:plan") == f"{cfg.name}:{plan_name}":
+                try:
+                    return int(row["dram_bytes_per_launch"])
+                except (KeyError, ValueError):
+                    return None
     return None
 
 

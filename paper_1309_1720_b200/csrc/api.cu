@@ -320,7 +320,9 @@ int cardiac_set_plan(cardiac_ctx* c, int plan, int param) {
   const bool rk_like = integ == I_EULER || integ == I_HEUN || integ == I_RK4;
   if (plan == CARDIAC_PLAN_AUTO) resolved = auto_plan(c->pb);
   if (resolved == CARDIAC_PLAN_STAGE) {
-    if (param != 0) return fail(c, CARDIAC_ERR_INVALID, "plan parameter must be 0");
+    if (param < 0 || param > 2)
+      return fail(c, CARDIAC_ERR_INVALID, "STAGE: parameter must be 0 (auto), 1 (direct) or 2 (TMA ring)");
+    rparam = param;
   } else if (resolved == CARDIAC_PLAN_FUSED) {
     if (!rk_like) return fail(c, CARDIAC_ERR_INVALID, "FUSED supports Euler, Heun and RK4 only");
     if (integ == I_EULER) {
@@ -336,6 +338,7 @@ int cardiac_set_plan(cardiac_ctx* c, int plan, int param) {
   c->plan_req = plan;
   c->plan = resolved;
   c->plan_param = rparam;
+  c->pb.stage_impl = resolved == CARDIAC_PLAN_STAGE ? rparam : 0;
   drop_graphs(c);
   return CARDIAC_OK;
 }

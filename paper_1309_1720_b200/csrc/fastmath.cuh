@@ -29,6 +29,26 @@ __constant__ double kExpC[12] = {
     1.0 / 362880.0,     1.0 / 40320.0,     1.0 / 5040.0,     1.0 / 720.0,
     1.0 / 120.0,        1.0 / 24.0,        1.0 / 6.0,        0.5};
 
+// clamp(t, 0, 1) and clamp(x, -700, 700) decided on the HIGH WORD with integer instructions.
+// fmin/fmax on doubles have no single sm_100a instruction: each expands to DSETP (on the FP64 pipe)
+// + SEL + FSEL + a NaN-quieting LOP3 + moves (~7 instructions; the BOCF reaction has 14 of them per
+// cell, a quarter of its v2 instruction count).  A double with the sign bit set is < 0 (or -0) and a
+// non-negative double is >= 1 iff its high word is >= 0x3FF00000, so ONE unsigned compare decides
+// "outside [0, 1)"; the replacement value is 0 or 1 by the sign.  Same results as fmin(fmax(t,0),1)
+// for every non-NaN t (-0 -> +0); NaN -> 0 or 1 by its sign (a NaN state is already lost).
+CARDIAC_D double clamp01(double t) {
+  const int hi = __double2hiint(t);
+  const bool out = (unsigned)hi >= 0x3FF00000u;
+  const int alt = ~(hi >> 31) & 0x3FF00000;   // t < 0 -> 0.0, t >= 1 -> 1.0
+  return __hiloint2double(out ? alt : hi, out ? 0 : __double2loint(t));
+}
+// |x| >= 700 <=> (high word & 0x7FFFFFFF) >= 0x4085E000 (700.0 = 0x4085E000'00000000)
+CARDIAC_D double clamp700(double x) {
+  const int hi = __double2hiint(x);
+  const bool out = (hi & 0x7FFFFFFF) >= 0x4085E000;
+  return __hiloint2double(out ? ((hi & 0x80000000) | 0x4085E000) : hi, out ? 0 : __double2loint(x));
+}
+
 // b > 0, normal range
 CARDIAC_D double rcp_pos(double b) {
   double r;
@@ -44,7 +64,7 @@ CARDIAC_D double exp_c(double x) {
   const double kLn2Hi = 0.6931471787393093;       // ln2 with the low 24 mantissa bits zero: n*hi exact
   const double kLn2Lo = 1.8206359985041462e-09;   // ln2 - kLn2Hi (60-digit ln2)
   const double kMagic = 6755399441055744.0;       // 1.5 * 2^52: fma(x, c, magic) rounds x c to an integer
-  x = fmin(fmax(x, -700.0), 700.0);
+  x = clamp700(x);
   double t = fma(x, kL2E, kMagic);
   int n = __double2loint(t);
   double fn = t - kMagic;

@@ -24,7 +24,7 @@ enum { V_PAPER = 0, V_TANHFREE = 1 };
 // H_k(x) = t^2 (3 - 2t), t = clamp(k x + 1/2, 0, 1): PAPER.md:94 (its branch form, Q11).
 CARDIAC_D double hk(double x, double k) {
   double t = fma(k, x, 0.5);
-  t = fmin(fmax(t, 0.0), 1.0);
+  t = clamp01(t);
   return t * t * fma(-2.0, t, 3.0);
 }
 

@@ -13,6 +13,7 @@ struct Problem {
   long long bstride;    // doubles per batch member
   double dx, dt;
   double params[32];    // public parameter block (include/cardiac.h)
+  int stage_impl;       // plan STAGE: 0 = pick by size, 1 = DIRECT (stage_kernels.cu), 2 = RING (stream_kernels.cu)
 };
 
 // One stage launch of the STAGE plan (kind = K_* of stage.cuh).
@@ -28,6 +29,11 @@ struct StageLaunch {
 
 // stage_kernels.cu: fused stencil + reaction + RK-stage combine, one launch per substep.
 cudaError_t launch_stage(const Problem& pb, const StageLaunch& st, cudaStream_t stream);
+
+// stream_kernels.cu: the same stage update fed by a TMA ring (persistent CTAs); K_SELF/K_BASE/K_RK4F
+bool stage_ring_supported(const Problem& pb, int kind);
+cudaError_t launch_stage_ring(const Problem& pb, const StageLaunch& st, cudaStream_t stream);
+constexpr long long kRingMinCells = 1 << 20;  // AUTO: below this the persistent grid has too few tiles per CTA
 
 // jvp: J[b-1] = (Z[b] - Z[0]) / eps, pitched state -> dense output
 cudaError_t launch_jvp(const Problem& pb, const double* state, double eps, double* dst_dense,

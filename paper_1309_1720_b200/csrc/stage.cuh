@@ -80,6 +80,35 @@ struct Stencil<S_BOX9> {
   }
 };
 
+// 128-bit accesses of an x-adjacent pair of cells ("vector width 2 for doubles")
+CARDIAC_D double2 ld2(const double* p) { return *reinterpret_cast<const double2*>(p); }
+CARDIAC_D void st2(double* p, double a, double b) { *reinterpret_cast<double2*>(p) = make_double2(a, b); }
+
+// integer-weight stencil sums of the two cells (x, x+1) of row `row`; interior, no boundary logic
+template <int STENCIL>
+CARDIAC_D void stencil_pair(const double* __restrict__ U, int row, int x, int pitch, double2 c,
+                            double& s0, double& s1) {
+  const double* p = U + row + x;
+  if (STENCIL == S_LAP5) {
+    const double w = p[-1], e = p[2];
+    const double2 s = ld2(p - pitch), n = ld2(p + pitch);
+    s0 = Stencil<S_LAP5>::apply(c.x, w, c.y, s.x, n.x);
+    s1 = Stencil<S_LAP5>::apply(c.y, c.x, e, s.y, n.y);
+  } else if (STENCIL == S_LAP9X4) {
+    const double2 l = ld2(p - 2), r = ld2(p + 2);
+    const double2 a1 = ld2(p - pitch), b1 = ld2(p + pitch);
+    const double2 a2 = ld2(p - 2 * pitch), b2 = ld2(p + 2 * pitch);
+    s0 = Stencil<S_LAP9X4>::apply(c.x, l.y, c.y, a1.x, b1.x, l.x, r.x, a2.x, b2.x);
+    s1 = Stencil<S_LAP9X4>::apply(c.y, c.x, r.x, a1.y, b1.y, l.y, r.y, a2.y, b2.y);
+  } else {
+    const double w = p[-1], e = p[2];
+    const double2 s = ld2(p - pitch), n = ld2(p + pitch);
+    const double sw = p[-pitch - 1], se = p[-pitch + 2], nw = p[pitch - 1], ne = p[pitch + 2];
+    s0 = Stencil<S_BOX9>::apply(c.x, w, c.y, s.x, n.x, sw, s.y, nw, n.y);
+    s1 = Stencil<S_BOX9>::apply(c.y, c.x, e, s.y, n.y, s.x, se, n.x, ne);
+  }
+}
+
 // the RK combination of one field value, shared by every plan
 template <int KIND>
 CARDIAC_D double combine(double w_y, double w_in, double w_A, double w_B, double w_f, double y,

@@ -21,34 +21,6 @@ namespace {
 
 constexpr int TX = 32, TY = 8;   // threads; the tile is 2*TX x TY cells
 
-CARDIAC_D double2 ld2(const double* p) { return *reinterpret_cast<const double2*>(p); }
-CARDIAC_D void st2(double* p, double a, double b) { *reinterpret_cast<double2*>(p) = make_double2(a, b); }
-
-// integer-weight stencil sums of the two cells (x, x+1) of row `row`; interior, no boundary logic
-template <int STENCIL>
-CARDIAC_D void stencil_pair(const double* __restrict__ U, int row, int x, int pitch, double2 c,
-                            double& s0, double& s1) {
-  const double* p = U + row + x;
-  if (STENCIL == S_LAP5) {
-    const double w = p[-1], e = p[2];
-    const double2 s = ld2(p - pitch), n = ld2(p + pitch);
-    s0 = Stencil<S_LAP5>::apply(c.x, w, c.y, s.x, n.x);
-    s1 = Stencil<S_LAP5>::apply(c.y, c.x, e, s.y, n.y);
-  } else if (STENCIL == S_LAP9X4) {
-    const double2 l = ld2(p - 2), r = ld2(p + 2);
-    const double2 a1 = ld2(p - pitch), b1 = ld2(p + pitch);
-    const double2 a2 = ld2(p - 2 * pitch), b2 = ld2(p + 2 * pitch);
-    s0 = Stencil<S_LAP9X4>::apply(c.x, l.y, c.y, a1.x, b1.x, l.x, r.x, a2.x, b2.x);
-    s1 = Stencil<S_LAP9X4>::apply(c.y, c.x, r.x, a1.y, b1.y, l.y, r.y, a2.y, b2.y);
-  } else {
-    const double w = p[-1], e = p[2];
-    const double2 s = ld2(p - pitch), n = ld2(p + pitch);
-    const double sw = p[-pitch - 1], se = p[-pitch + 2], nw = p[pitch - 1], ne = p[pitch + 2];
-    s0 = Stencil<S_BOX9>::apply(c.x, w, c.y, s.x, n.x, sw, s.y, nw, n.y);
-    s1 = Stencil<S_BOX9>::apply(c.y, c.x, e, s.y, n.y, s.x, se, n.x, ne);
-  }
-}
-
 // one cell with the boundary rule applied per axis (Q3)
 template <int STENCIL>
 CARDIAC_D double stencil_edge(const double* __restrict__ U, int i, int j, int nx, int ny, int pitch,
@@ -108,7 +80,7 @@ CARDIAC_D void finish_cell(const StageArgs<MD>& a, const double* __restrict__ yb
 }
 
 template <class MD, int STENCIL, int KIND>
-__global__ void __launch_bounds__(TX* TY)
+__global__ void __launch_bounds__(TX* TY, 4)
     stage_kernel(const __grid_constant__ StageArgs<MD> a) {
   constexpr int NV = MD::NV, ND = MD::ND;
   constexpr int R = stencil_radius(STENCIL);
@@ -129,18 +101,14 @@ __global__ void __launch_bounds__(TX* TY)
     double2 zz[NV];
 #pragma unroll
     for (int q = 0; q < NV; ++q) zz[q] = ld2(in + o + q * a.g.fstride);
-    double2 yy[NV] = {}, AA[NV] = {}, BB[NV] = {};
-    if (KIND != K_SELF) {
+    // Stencil first: its neighbour loads go out together with the centre loads and are reduced to
+    // two sums per diffusing field before the (register-hungry) reaction starts.  The RK operands
+    // y / Y2 / Y3 are loaded after it, next to their use: with the kernel held to 64 registers
+    // (4 blocks = 32 warps per SM) the other warps cover that second latency, which measured faster
+    // than keeping 12 more 128-bit loads in flight per thread (or prefetching them to L1).
+    double s0[ND], s1[ND];
 #pragma unroll
-      for (int q = 0; q < NV; ++q) yy[q] = ld2(yb + o + q * a.g.fstride);
-    }
-    if (KIND == K_RK4F) {
-#pragma unroll
-      for (int q = 0; q < NV; ++q) {
-        AA[q] = ld2(Ab + o + q * a.g.fstride);
-        BB[q] = ld2(Bb + o + q * a.g.fstride);
-      }
-    }
+    for (int q = 0; q < ND; ++q) stencil_pair<STENCIL>(in + q * a.g.fstride, row, x, pitch, zz[q], s0[q], s1[q]);
     double z0[NV], z1[NV], f0[NV], f1[NV];
 #pragma unroll
     for (int q = 0; q < NV; ++q) { z0[q] = zz[q].x; z1[q] = zz[q].y; }
@@ -148,15 +116,16 @@ __global__ void __launch_bounds__(TX* TY)
     MD::reaction(a.p, z1, f1);
 #pragma unroll
     for (int q = 0; q < ND; ++q) {
-      double s0, s1;
-      stencil_pair<STENCIL>(in + q * a.g.fstride, row, x, pitch, zz[q], s0, s1);
-      f0[q] = fma(a.lapw[q], s0, f0[q]);
-      f1[q] = fma(a.lapw[q], s1, f1[q]);
+      f0[q] = fma(a.lapw[q], s0[q], f0[q]);
+      f1[q] = fma(a.lapw[q], s1[q], f1[q]);
     }
 #pragma unroll
     for (int q = 0; q < NV; ++q) {
-      double r0 = combine<KIND>(a.w_y, a.w_in, a.w_A, a.w_B, a.w_f, yy[q].x, z0[q], AA[q].x, BB[q].x, f0[q]);
-      double r1 = combine<KIND>(a.w_y, a.w_in, a.w_A, a.w_B, a.w_f, yy[q].y, z1[q], AA[q].y, BB[q].y, f1[q]);
+      double2 yy = make_double2(0.0, 0.0), AA = yy, BB = yy;
+      if (KIND != K_SELF) yy = ld2(yb + o + q * a.g.fstride);
+      if (KIND == K_RK4F) { AA = ld2(Ab + o + q * a.g.fstride); BB = ld2(Bb + o + q * a.g.fstride); }
+      double r0 = combine<KIND>(a.w_y, a.w_in, a.w_A, a.w_B, a.w_f, yy.x, z0[q], AA.x, BB.x, f0[q]);
+      double r1 = combine<KIND>(a.w_y, a.w_in, a.w_A, a.w_B, a.w_f, yy.y, z1[q], AA.y, BB.y, f1[q]);
       st2(ob + o + q * a.g.fstride, r0, r1);
     }
     return;
@@ -242,6 +211,15 @@ __global__ void jvp_kernel(const double* __restrict__ Z, double* __restrict__ J,
 }  // namespace
 
 cudaError_t launch_stage(const Problem& pb, const StageLaunch& st, cudaStream_t stream) {
+  // DIRECT vs RING (bitwise identical results).  Measured on B200 (profiles/, r1 v4): with 32 warps
+  // per SM the direct kernels hide their own load latency and win wherever a stage is bound by the
+  // FP64 pipe or moves few bytes per cell; the TMA ring wins on the one stage that is purely
+  // HBM-bound and operand-heavy — the last RK4 stage of the 4-field model (16 doubles in, 4 out per
+  // cell; 6.3 TB/s = 96 % of the measured copy bandwidth, against 5.9 TB/s direct).
+  const long long cells = (long long)pb.nx * pb.ny * pb.batch;
+  const bool ring_auto = st.kind == K_RK4F && pb.nv >= 4 && cells >= kRingMinCells;
+  if (pb.stage_impl != 1 && (pb.stage_impl == 2 || ring_auto) && stage_ring_supported(pb, st.kind))
+    return launch_stage_ring(pb, st, stream);
   if (pb.model == M_FHN) return by_stencil<Model<M_FHN, V_PAPER>>(pb, st, stream);
   if (pb.model == M_KARMA)
     return pb.variant == V_TANHFREE ? by_stencil<Model<M_KARMA, V_TANHFREE>>(pb, st, stream)

@@ -28,6 +28,8 @@ def C():
 
 
 def gpu_run(C, cfg, Z0, nsteps, plan=0, plan_param=0, params=None, chunks=None):
+    if isinstance(plan, tuple):          # (CARDIAC_PLAN_*, plan parameter)
+        plan, plan_param = plan
     with C.Context.from_config(cfg, plan=plan, plan_param=plan_param, params=params) as ctx:
         ctx.set_state(np.ascontiguousarray(Z0))
         for n in (chunks or [nsteps]):
@@ -52,8 +54,11 @@ CASES = [(m, s, i) for m in (FHN, KARMA, BOCF) for s in (LAP5, LAP9X4, BOX9) for
 CASES += [(BOCF, s, i) for s in (LAP5, LAP9X4, BOX9) for i in (RL, IE)]
 
 
-STAGE, FUSED = 1, 2      # CARDIAC_PLAN_*
-PLAN_CASES = [(m, s, i, STAGE) for (m, s, i) in CASES] + [(m, s, i, FUSED) for (m, s, i) in CASES if i in (EULER, HEUN, RK4)]
+# CARDIAC_PLAN_* (+ parameter): STAGE with its DIRECT kernels, STAGE with the TMA-ring kernels
+# (forced: AUTO would pick DIRECT at these oracle-sized grids), FUSED
+STAGE, RING, FUSED = (1, 1), (1, 2), 2
+PLAN_CASES = [(m, s, i, STAGE) for (m, s, i) in CASES]
+PLAN_CASES += [(m, s, i, p) for (m, s, i) in CASES if i in (EULER, HEUN, RK4) for p in (RING, FUSED)]
 
 
 @pytest.mark.parametrize("model,stencil,integ,plan", PLAN_CASES)
@@ -73,7 +78,7 @@ def test_parity_one_and_hundred_steps(C, model, stencil, integ, plan):
 
 @pytest.mark.parametrize("model,stencil,integ", [(FHN, LAP9X4, RK4), (KARMA, LAP5, RK4), (BOCF, LAP9X4, RK4),
                                                  (FHN, LAP5, EULER), (BOCF, BOX9, HEUN)])
-@pytest.mark.parametrize("plan", [STAGE, FUSED])
+@pytest.mark.parametrize("plan", [STAGE, RING, FUSED])
 def test_parity_periodic_boundary(C, model, stencil, integ, plan):
     cfg, Z = make(model, 37, 50, stencil, integ, boundary=1)
     got = gpu_run(C, cfg, Z, 30, plan=plan)
@@ -82,7 +87,7 @@ def test_parity_periodic_boundary(C, model, stencil, integ, plan):
 
 
 @pytest.mark.parametrize("model", [KARMA, BOCF])
-@pytest.mark.parametrize("plan", [STAGE, FUSED])
+@pytest.mark.parametrize("plan", [STAGE, RING, FUSED])
 def test_parity_tanhfree_variant(C, model, plan):
     cfg, Z = make(model, 40, 33, LAP9X4, RK4, variant=1)
     got = gpu_run(C, cfg, Z, 50, plan=plan)
@@ -94,7 +99,7 @@ def test_parity_tanhfree_variant(C, model, plan):
 
 @pytest.mark.parametrize("model,stencil,nx,ny", [(FHN, LAP5, 3, 3), (FHN, LAP9X4, 5, 5), (KARMA, LAP9X4, 5, 64),
                                                  (BOCF, LAP5, 200, 3), (FHN, BOX9, 3, 17), (KARMA, LAP5, 33, 4)])
-@pytest.mark.parametrize("plan", [STAGE, FUSED])
+@pytest.mark.parametrize("plan", [STAGE, RING, FUSED])
 def test_parity_degenerate_sizes(C, model, stencil, nx, ny, plan):
     """Minimum sizes 2r+1 (every stencil arm reflects; the fused window folds the grid several
     times over) and thin strips."""
@@ -104,7 +109,7 @@ def test_parity_degenerate_sizes(C, model, stencil, nx, ny, plan):
     assert maxabs(got, ref) <= TOL_100
 
 
-@pytest.mark.parametrize("plan", [STAGE, FUSED])
+@pytest.mark.parametrize("plan", [STAGE, RING, FUSED])
 def test_batch_members_independent_of_position(C, plan):
     cfg, Z = make(KARMA, 48, 40, LAP5, RK4, batch=5, seed=3)
     def gpu_run_p(C, cfg, Z, n):
@@ -121,6 +126,7 @@ def test_batch_members_independent_of_position(C, plan):
 
 
 @pytest.mark.parametrize("model,integ,plan", [(FHN, EULER, STAGE), (FHN, RK4, STAGE), (KARMA, HEUN, STAGE),
+                                              (FHN, EULER, RING), (BOCF, RK4, RING), (KARMA, HEUN, RING),
                                               (BOCF, RL, STAGE), (FHN, EULER, FUSED), (FHN, RK4, FUSED),
                                               (KARMA, HEUN, FUSED), (BOCF, EULER, FUSED)])
 def test_step_composition_and_determinism_bitwise(C, model, integ, plan):
@@ -142,7 +148,10 @@ def test_fused_many_tiles_matches_stage_plan_and_oracle(C):
         got = gpu_run(C, cfg, Z, 12, plan=FUSED)
         ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 12)
         assert maxabs(got, ref) <= TOL_100
-        assert maxabs(got, gpu_run(C, cfg, Z, 12, plan=STAGE)) <= 1e-12
+        direct = gpu_run(C, cfg, Z, 12, plan=STAGE)
+        assert maxabs(got, direct) <= 1e-12
+        # the TMA-ring kernels run the same arithmetic per cell as the direct ones: bitwise equal
+        assert np.array_equal(gpu_run(C, cfg, Z, 12, plan=RING), direct)
 
 
 def test_plan_switch_keeps_state(C):
@@ -150,7 +159,7 @@ def test_plan_switch_keeps_state(C):
     with C.Context.from_config(cfg, plan=FUSED) as ctx:
         ctx.set_state(Z)
         ctx.step(3)                                   # odd number of ping-pong launches
-        C.cardiac_set_plan(ctx.ctx, STAGE, 0)
+        C.cardiac_set_plan(ctx.ctx, *STAGE)
         ctx.step(4)
         C.cardiac_set_plan(ctx.ctx, FUSED, 0)
         ctx.step(2)
@@ -199,7 +208,7 @@ def test_error_paths_and_device_buffers(C):
     cfg, Z = make(FHN, 40, 30, LAP5, EULER)
     ctx = C.cardiac_create(cfg.model, cfg.nx, cfg.ny, cfg.dx, cfg.dt, cfg.scheme, 1)
     try:
-        C.cardiac_set_plan(ctx, STAGE, 0)        # one launch per Euler step: launch counts below
+        C.cardiac_set_plan(ctx, *STAGE)        # one launch per Euler step: launch counts below
         with pytest.raises(C.CardiacError) as ei:
             C.cardiac_step(ctx, 1)
         assert ei.value.code == C.CARDIAC_ERR_NOSTATE

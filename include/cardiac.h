@@ -68,8 +68,10 @@ enum {
   CARDIAC_PLAN_STAGE      = 1, /* one fused stencil+reaction+RK-stage launch per substep        */
   CARDIAC_PLAN_FUSED      = 2, /* all substeps of one time step (or several Euler steps) on chip,
                                   overlapped tiles, one launch                                  */
-  CARDIAC_PLAN_PERSISTENT = 3  /* one cooperative launch for all nsteps; tiles resident on chip,
-                                  neighbour halo exchange through L2                            */
+  CARDIAC_PLAN_PERSISTENT = 3  /* ONE launch for all nsteps: each batch member resident in the shared
+                                  memory of a thread-block cluster (<= 8 CTAs), ghost rows exchanged
+                                  through distributed shared memory; grids up to 8 x 4096 cells
+                                  (4-field model: 8 x 2048); Euler, Heun, RK4                   */
 };
 
 /* error codes */

@@ -80,6 +80,8 @@ void carve(cardiac_ctx* c) {
 // (DESIGN.md "Plans").
 int auto_plan(const Problem& pb) {
   const bool rk_like = pb.integrator == I_EULER || pb.integrator == I_HEUN || pb.integrator == I_RK4;
+  // a grid that fits one SM never leaves it: the paper's launch-bound regime N < N0
+  if (resident_preferred(pb)) return CARDIAC_PLAN_PERSISTENT;
   if (rk_like && pb.model != CARDIAC_BOCF) return CARDIAC_PLAN_FUSED;
   return CARDIAC_PLAN_STAGE;
 }
@@ -332,6 +334,11 @@ int cardiac_set_plan(cardiac_ctx* c, int plan, int param) {
     } else if (param != 0) {
       return fail(c, CARDIAC_ERR_INVALID, "plan parameter must be 0");
     }
+  } else if (resolved == CARDIAC_PLAN_PERSISTENT) {
+    if (!resident_supported(c->pb))
+      return fail(c, CARDIAC_ERR_INVALID,
+                  "PERSISTENT needs Euler/Heun/RK4 and a grid that fits one cluster: 8 x 4096 cells (4-field model: 8 x 2048)");
+    if (param != 0) return fail(c, CARDIAC_ERR_INVALID, "plan parameter must be 0");
   } else {
     return fail(c, CARDIAC_ERR_INVALID, "plan not available for this context");
   }
@@ -400,6 +407,13 @@ int cardiac_step(cardiac_ctx* c, long long nsteps) {
   if (!c->has_state) return fail(c, CARDIAC_ERR_NOSTATE, "no state set");
   if (nsteps == 0) return CARDIAC_OK;
   DeviceGuard guard(c->device);
+  if (c->plan == CARDIAC_PLAN_PERSISTENT) {   // one launch, in place, whatever nsteps
+    ResidentLaunch rl{c->buf[c->cur], nsteps};
+    cudaError_t e = launch_resident(c->pb, rl, c->stream);
+    if (e != cudaSuccess) return fail_cuda(c, e, "resident launch");
+    c->launches++;
+    return CARDIAC_OK;
+  }
   const int us = unit_steps(c);                                        // time steps per unit
   const int ul = c->plan == CARDIAC_PLAN_FUSED ? 1 : stages_of(c->pb.integrator);  // launches per unit
   int gunits = kGraphNodes / ul;

@@ -56,6 +56,53 @@ inline cudaError_t launch_fused(const Problem& pb, const TileLaunch& tl, cudaStr
                                         : launch_fused_bocf(pb, tl, stream));
 }
 
+// resident_kernels_*.cu: plan PERSISTENT — one thread-block cluster of C <= 8 CTAs per batch member
+// keeps the whole grid in (distributed) shared memory and advances all nsteps in ONE launch, in place
+// (resident.cuh).  C CTAs of 512 threads x KP pairs: at most C x 4096 cells (2-field models) or
+// C x 2048 cells (4-field model); Euler / Heun / RK4.
+struct ResidentLaunch {
+  double* state;
+  long long nsteps;
+};
+struct ResidentShape {
+  int csize;   // CTAs per cluster (power of two, 0 = does not fit)
+  int slab;    // rows per CTA
+  size_t smem; // dynamic shared memory per CTA
+};
+inline ResidentShape resident_shape(const Problem& pb) {
+  ResidentShape rs{0, 0, 0};
+  if (pb.integrator > 2) return rs;  // Euler, Heun, RK4
+  const long long npx = (pb.nx + 1) / 2, cap = 512LL * (pb.nv > 2 ? 2 : 4);
+  const size_t sp = 2 * (size_t)npx + 4;
+  for (int c = 1; c <= 8; c *= 2) {
+    const int slab = (pb.ny + c - 1) / c;
+    const size_t smem = 2 * (size_t)pb.nd * sp * ((size_t)slab + 2 * pb.radius) * sizeof(double);
+    // fits, and one pair per thread where the grid is large enough to spread (the substep is
+    // bound by the barrier, not by arithmetic, below that)
+    if (npx * slab <= cap && smem <= 200 * 1024 && (npx * slab <= 512 || c == 8)) {
+      rs.csize = c; rs.slab = slab; rs.smem = smem;
+      return rs;
+    }
+  }
+  return rs;
+}
+inline bool resident_supported(const Problem& pb) { return resident_shape(pb).csize > 0; }
+// AUTO: measured on B200, one cluster-resident launch beats the per-step
+// launches of FUSED / STAGE up to about 100 x 100 cells per member (a substep costs ~1 us of
+// barrier + ghost exchange whatever the size), as long as the batch does not already fill the GPU
+inline bool resident_preferred(const Problem& pb) {
+  const ResidentShape rs = resident_shape(pb);
+  return rs.csize > 0 && (long long)((pb.nx + 1) / 2) * pb.ny <= 5120 && (long long)pb.batch * rs.csize <= 296;
+}
+cudaError_t launch_resident_fhn(const Problem& pb, const ResidentLaunch& rl, cudaStream_t stream);
+cudaError_t launch_resident_karma(const Problem& pb, const ResidentLaunch& rl, cudaStream_t stream);
+cudaError_t launch_resident_bocf(const Problem& pb, const ResidentLaunch& rl, cudaStream_t stream);
+inline cudaError_t launch_resident(const Problem& pb, const ResidentLaunch& rl, cudaStream_t stream) {
+  return pb.model == 0 ? launch_resident_fhn(pb, rl, stream)
+                       : (pb.model == 1 ? launch_resident_karma(pb, rl, stream)
+                                        : launch_resident_bocf(pb, rl, stream));
+}
+
 // probe_kernels.cu: diagnostic evaluation of the device math / reactions on sample points
 enum { PROBE_EXP = 0, PROBE_RCP = 1, PROBE_HK = 2, PROBE_REACTION = 3 };
 cudaError_t launch_probe(const Problem& pb, int what, const double* in, double* out, long long n,

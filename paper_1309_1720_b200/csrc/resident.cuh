@@ -1,0 +1,277 @@
+// resident.cuh — plan PERSISTENT for grids that fit the shared memory of one thread-block cluster:
+// ONE launch advances all nsteps.
+//
+// The paper's small-grid regime (N < N0 ~ 362, Fig. 5 :166) is bound by the cost of
+// launching (n_d + 2) n_s kernels per time step, not by arithmetic.  Here a batch member is owned
+// by one cluster of C <= 8 CTAs for the whole run; CTA `rank` holds the slab of rows
+// [rank h, rank h + h).  The stage values of the diffusing fields live in two shared-memory buffers
+// framed by a ghost ring of r cells, each thread owns up to KP fixed x-adjacent pairs of cells and
+// keeps their step-start value y, the running RK sum and the gating variables in registers.
+// A substep is: stencil + reaction + RK update of the owned cells (buffer `cur` -> `nxt`),
+// cluster barrier, refill of the ghost ring of `nxt` — ghost columns from the CTA's own rows, ghost
+// rows from the shared memory of the CTA that owns the row the index reflects / wraps / continues
+// to, read through distributed shared memory (PAPER.md:104 Fig. 1, :114; Q3) — CTA
+// barrier.  Global memory is touched before the first and after the last step only; the
+// "lock-step" between substeps is a hardware cluster barrier (~0.2 us) instead of a
+// kernel boundary.  Batch members (the nearby trajectories of a Newton-Krylov solve)
+// run on different clusters.
+//
+// The per-cell arithmetic is the instruction sequence of the tile engine (tile.cuh): same
+// Stencil<>::apply operand pairing, Model<>::reaction, a_dt / b_dt updates — results are bitwise
+// those of plan FUSED.
+#pragma once
+#include "stage.cuh"
+#include "tile.cuh"
+
+namespace cardiac {
+
+constexpr int kResidentThreads = 512;
+constexpr int kResidentMaxCluster = 8;   // portable cluster size
+
+template <class MD>
+struct ResidentArgs {
+  const double* in;
+  double* out;
+  Geom g;
+  long long nsteps;
+  int npx;         // pairs per row = ceil(nx / 2)
+  int slab;        // rows per CTA = ceil(ny / C)
+  int csize;       // C, CTAs per cluster = per batch member
+  int sp, sr;      // shared row pitch (doubles, even) and rows per field: 2 npx + 4, slab + 2 r
+  double a_dt[4], b_dt[4];
+  double lapw[MD::ND];
+  typename MD::Params p;
+};
+
+CARDIAC_D unsigned cluster_rank() {
+  unsigned r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+CARDIAC_D void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// the value at the same shared-memory offset as `p` in CTA `rank` of the cluster
+CARDIAC_D double ld_cluster(const double* p, unsigned rank) {
+  unsigned local = (unsigned)__cvta_generic_to_shared(p), remote;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local), "r"(rank));
+  double v;
+  asm volatile("ld.shared::cluster.f64 %0, [%1];" : "=d"(v) : "r"(remote) : "memory");
+  return v;
+}
+
+template <class MD, int STENCIL, int INTEG, int KP>
+struct ResidentEngine {
+  static constexpr int NV = MD::NV, ND = MD::ND, NG = NV - ND;
+  static constexpr int R = stencil_radius(STENCIL);
+  static constexpr int NS = StepScheme<INTEG, 1>::NS;
+  static constexpr bool RK = StepScheme<INTEG, 1>::RK;
+  static constexpr int NT = kResidentThreads;
+  static constexpr int GX = 2;  // ghost columns kept on each side (>= r; keeps pairs 16-byte aligned)
+
+  static constexpr int GK = 2;  // ghost cells per thread decoded once
+  struct Ghost;
+  struct Patch;
+
+
+  // The ghost ring of the slab [y0, y0 + rows): ghost columns -r..-1, nx..nx+r-1 of the own rows
+  // (source: the own row, reflected / wrapped column) and ghost rows y0-r..y0-1, y0+rows..y0+rows+r-1
+  // over the columns 0..nx-1 (source: the CTA that owns the grid row the index stands for).
+  // Entry e of that list -> offset of the ghost cell inside buffer 0, offset of its source, owner.
+  struct Ghost {
+    int dst, src;
+    unsigned owner;
+  };
+  struct Patch {
+    double y[RK ? KP : 1][2][NV];
+    double acc[RK ? KP : 1][2][NV];
+    double g[KP][2][NG > 0 ? NG : 1];
+    int off[KP];   // offset of the pair inside a shared field, -1 = no such pair
+    Ghost gh[GK];  // dst < 0: none
+  };
+  CARDIAC_D static Ghost ghost_entry(const ResidentArgs<MD>& a, int e, int y0, int rows, unsigned rank) {
+    const int nx = a.g.nx, ny = a.g.ny, bc = a.g.boundary, sp = a.sp;
+    const int ncol = 2 * R * rows, nrow = 2 * R * nx;
+    const int q = e / (ncol + nrow), f = e - q * (ncol + nrow);
+    const int fo = q * a.sp * a.sr;
+    Ghost gh;
+    if (f < ncol) {
+      const int k = f / rows, lr = f - k * rows + R;
+      const int gx = k < R ? -1 - k : nx + (k - R);
+      gh.dst = fo + lr * sp + GX + gx;
+      gh.src = fo + lr * sp + GX + bidx(gx, nx, bc);
+      gh.owner = rank;
+    } else {
+      const int h = f - ncol, k = h / nx, gx = h - k * nx;
+      const int gy = k < R ? y0 - 1 - k : y0 + rows + (k - R);
+      const int gs = bidx(gy, ny, bc);          // the grid row it stands for
+      gh.owner = (unsigned)(gs / a.slab);
+      gh.dst = fo + (gy - y0 + R) * sp + GX + gx;
+      gh.src = fo + (gs - (int)gh.owner * a.slab + R) * sp + GX + gx;
+    }
+    return gh;
+  }
+
+  // Refill the ghost ring of buffer `b`.  Call after a cluster barrier (the interior of `b` is
+  // complete in every CTA); ends with a CTA barrier.  The first GK entries of every thread were
+  // decoded once (Patch::gh); longer lists (very wide grids) are decoded on the fly.
+  CARDIAC_D static void fill_ghosts(const ResidentArgs<MD>& a, double* __restrict__ b, int y0, int rows,
+                                    unsigned rank, const Patch& st) {
+    const int nghost = rows > 0 ? ND * 2 * R * (rows + a.g.nx) : 0;
+#pragma unroll
+    for (int k = 0; k < GK; ++k)
+      if (st.gh[k].dst >= 0) b[st.gh[k].dst] = ld_cluster(b + st.gh[k].src, st.gh[k].owner);
+    for (int e = threadIdx.x + GK * NT; e < nghost; e += NT) {
+      const Ghost gh = ghost_entry(a, e, y0, rows, rank);
+      b[gh.dst] = ld_cluster(b + gh.src, gh.owner);
+    }
+    __syncthreads();
+    if (STENCIL == S_BOX9) {   // corners: ghost columns of the ghost rows
+      const int nx = a.g.nx, bc = a.g.boundary, sp = a.sp, fsz = a.sp * a.sr;
+      for (int e = threadIdx.x; e < ND * 2 * R * 2 * R && rows > 0; e += NT) {
+        const int q = e / (4 * R * R), f = e - q * 4 * R * R, kr = f / (2 * R), kc = f - kr * 2 * R;
+        const int lr = kr < R ? R - 1 - kr : R + rows + (kr - R);
+        const int gx = kc < R ? -1 - kc : nx + (kc - R);
+        double* F = b + q * fsz;
+        F[lr * sp + GX + gx] = F[lr * sp + GX + bidx(gx, nx, bc)];
+      }
+      __syncthreads();
+    }
+  }
+
+  // Substep S of every owned pair: reads `cur`, writes the diffusing fields of `nxt`.
+  template <int S>
+  CARDIAC_D static void stage(const ResidentArgs<MD>& a, const double* __restrict__ cur,
+                              double* __restrict__ nxt, Patch& st) {
+    constexpr bool LAST = (S == NS - 1);
+    const int fsz = a.sp * a.sr;
+#pragma unroll
+    for (int k = 0; k < KP; ++k) {
+      const int o = st.off[k];
+      if (o < 0) break;
+      double2 ctr[ND];
+      double s0[ND], s1[ND];
+#pragma unroll
+      for (int q = 0; q < ND; ++q) {
+        ctr[q] = ld2(cur + q * fsz + o);
+        stencil_pair<STENCIL>(cur + q * fsz, o, 0, a.sp, ctr[q], s0[q], s1[q]);
+      }
+      double res[2][NV];
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        double z[NV], f[NV];
+#pragma unroll
+        for (int q = 0; q < NV; ++q)
+          z[q] = q < ND ? (h == 0 ? ctr[q < ND ? q : 0].x : ctr[q < ND ? q : 0].y)
+                        : st.g[k][h][q >= ND ? q - ND : 0];
+        MD::reaction(a.p, z, f);
+#pragma unroll
+        for (int q = 0; q < ND; ++q) f[q] = fma(a.lapw[q], h == 0 ? s0[q] : s1[q], f[q]);
+#pragma unroll
+        for (int q = 0; q < NV; ++q) {
+          double nv;
+          if (!RK) {
+            nv = fma(a.a_dt[0], f[q], z[q]);
+          } else if (LAST) {
+            nv = fma(a.b_dt[S], f[q], S == 0 ? st.y[k][h][q] : st.acc[k][h][q]);
+            st.y[k][h][q] = nv;   // the next time step starts here
+          } else {
+            st.acc[k][h][q] = fma(a.b_dt[S], f[q], S == 0 ? st.y[k][h][q] : st.acc[k][h][q]);
+            nv = fma(a.a_dt[S], f[q], st.y[k][h][q]);
+          }
+          res[h][q] = nv;
+          if (q >= ND) st.g[k][h][q >= ND ? q - ND : 0] = nv;
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < ND; ++q) st2(nxt + q * fsz + o, res[0][q], res[1][q]);
+    }
+  }
+
+  template <int S>
+  CARDIAC_D static void stages_from(const ResidentArgs<MD>& a, double* __restrict__ sm, int& cur,
+                                    Patch& st, int y0, int rows, unsigned rank) {
+    if constexpr (S < NS) {
+      const int fsz = a.sp * a.sr;
+      double* c = sm + cur * ND * fsz;
+      double* n = sm + (cur ^ 1) * ND * fsz;
+      stage<S>(a, c, n, st);
+      cluster_sync_all();
+      fill_ghosts(a, n, y0, rows, rank, st);
+      cur ^= 1;
+      stages_from<S + 1>(a, sm, cur, st, y0, rows, rank);
+    }
+  }
+
+  // `in` / `out`: the batch member.  Every CTA of the cluster runs this with its own rank.
+  CARDIAC_D static void run(const ResidentArgs<MD>& a, const double* __restrict__ in,
+                            double* __restrict__ out, double* __restrict__ sm) {
+    const int nx = a.g.nx, pitch = a.g.pitch;
+    const unsigned rank = cluster_rank();
+    const int y0 = (int)rank * a.slab;
+    const int rows = max(0, min(a.slab, a.g.ny - y0));
+    const int fsz = a.sp * a.sr, npairs = a.npx * rows;
+    Patch st;
+    // load: diffusing fields -> shared buffer 0, gating fields and y -> registers
+#pragma unroll
+    for (int k = 0; k < KP; ++k) {
+      const int p = threadIdx.x + k * NT;
+      st.off[k] = -1;
+      if (p >= npairs) continue;
+      const int py = p / a.npx, px = p - py * a.npx, gx = 2 * px;
+      st.off[k] = (py + R) * a.sp + GX + gx;
+#pragma unroll
+      for (int q = 0; q < NV; ++q) {
+        const double* f = in + q * a.g.fstride + (long long)(y0 + py) * pitch + gx;
+        double2 v;
+        v.x = f[0];
+        v.y = gx + 1 < nx ? f[1] : 0.0;
+        if (q < ND) st2(sm + q * fsz + st.off[k], v.x, v.y);
+        else { st.g[k][0][q >= ND ? q - ND : 0] = v.x; st.g[k][1][q >= ND ? q - ND : 0] = v.y; }
+        if (RK) { st.y[k][0][q] = v.x; st.y[k][1][q] = v.y; }
+      }
+    }
+    {
+      const int nghost = rows > 0 ? ND * 2 * R * (rows + nx) : 0;
+#pragma unroll
+      for (int k = 0; k < GK; ++k) {
+        const int e = threadIdx.x + k * NT;
+        st.gh[k].dst = -1;
+        if (e < nghost) st.gh[k] = ghost_entry(a, e, y0, rows, rank);
+      }
+    }
+    cluster_sync_all();
+    fill_ghosts(a, sm, y0, rows, rank, st);
+    int cur = 0;
+    for (long long n = 0; n < a.nsteps; ++n) stages_from<0>(a, sm, cur, st, y0, rows, rank);
+    // store the state: diffusing fields from the current shared buffer, gates from registers
+    const double* c = sm + cur * ND * fsz;
+#pragma unroll
+    for (int k = 0; k < KP; ++k) {
+      const int p = threadIdx.x + k * NT;
+      if (p >= npairs) break;
+      const int py = p / a.npx, px = p - py * a.npx, gx = 2 * px;
+#pragma unroll
+      for (int q = 0; q < NV; ++q) {
+        double* f = out + q * a.g.fstride + (long long)(y0 + py) * pitch + gx;
+        double2 v;
+        if (q < ND) v = ld2(c + q * fsz + st.off[k]);
+        else v = make_double2(st.g[k][0][q >= ND ? q - ND : 0], st.g[k][1][q >= ND ? q - ND : 0]);
+        f[0] = v.x;
+        if (gx + 1 < nx) f[1] = v.y;
+      }
+    }
+    cluster_sync_all();   // nobody leaves while a neighbour may still read its shared memory
+  }
+};
+
+template <class MD, int STENCIL, int INTEG, int KP>
+__global__ void __launch_bounds__(kResidentThreads, 1)
+    resident_kernel(const __grid_constant__ ResidentArgs<MD> a) {
+  extern __shared__ double2 smem_resident[];
+  const long long base = (long long)(blockIdx.x / a.csize) * a.g.bstride;
+  ResidentEngine<MD, STENCIL, INTEG, KP>::run(a, a.in + base, a.out + base,
+                                              reinterpret_cast<double*>(smem_resident));
+}
+
+}  // namespace cardiac

@@ -1,0 +1,88 @@
+// resident_dispatch.cuh — host dispatch of plan PERSISTENT for one model; included by the per-model
+// resident_kernels_*.cu files so that the instantiations compile in parallel.
+#pragma once
+#include "plans.h"
+#include "resident.cuh"
+
+namespace cardiac {
+
+// pairs per thread: 4 (4096 cells per CTA) for the two-field models; the 4-field model keeps 11
+// doubles per cell in registers, so 2 (2048 cells)
+template <class MD>
+struct ResidentPairs {
+  static constexpr int KP = MD::NV > 2 ? 2 : 4;
+};
+
+template <class MD, int STENCIL, int INTEG>
+cudaError_t resident_run(const Problem& pb, const ResidentLaunch& rl, cudaStream_t stream) {
+  constexpr int KP = ResidentPairs<MD>::KP;
+  constexpr int R = stencil_radius(STENCIL);
+  auto kern = resident_kernel<MD, STENCIL, INTEG, KP>;
+  ResidentArgs<MD> a;
+  a.in = rl.state; a.out = rl.state;
+  a.g.nx = pb.nx; a.g.ny = pb.ny; a.g.pitch = pb.pitch; a.g.boundary = pb.boundary;
+  a.g.fstride = pb.fstride; a.g.bstride = pb.bstride;
+  a.nsteps = rl.nsteps;
+  const ResidentShape rs = resident_shape(pb);
+  if (rs.csize == 0) return cudaErrorInvalidValue;
+  a.npx = (pb.nx + 1) / 2;
+  a.slab = rs.slab;
+  a.csize = rs.csize;
+  a.sp = 2 * a.npx + 4;
+  a.sr = rs.slab + 2 * R;
+  const double dt = pb.dt;
+  for (int s = 0; s < 4; ++s) a.a_dt[s] = a.b_dt[s] = 0.0;
+  if (INTEG == I_RK4) {
+    a.a_dt[0] = 0.5 * dt; a.a_dt[1] = 0.5 * dt; a.a_dt[2] = dt;
+    a.b_dt[0] = dt / 6.0; a.b_dt[1] = dt / 3.0; a.b_dt[2] = dt / 3.0; a.b_dt[3] = dt / 6.0;
+  } else if (INTEG == I_HEUN) {
+    a.a_dt[0] = dt; a.b_dt[0] = 0.5 * dt; a.b_dt[1] = 0.5 * dt;
+  } else {
+    a.a_dt[0] = dt;
+  }
+  MD::derive(pb.params, a.p);
+  for (int q = 0; q < MD::ND; ++q) a.lapw[q] = a.p.D[q] * stencil_norm(STENCIL) / (pb.dx * pb.dx);
+  const size_t smem = rs.smem;
+  if ((long long)a.npx * rs.slab > (long long)kResidentThreads * KP) return cudaErrorInvalidValue;
+  static size_t configured = 0;  // per instantiation
+  if (smem > configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    configured = smem;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)pb.batch * rs.csize);
+  cfg.blockDim = dim3(kResidentThreads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = rs.csize;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, a);
+}
+
+template <class MD, int STENCIL>
+cudaError_t resident_by_integrator(const Problem& pb, const ResidentLaunch& rl, cudaStream_t s) {
+  switch (pb.integrator) {
+    case I_EULER: return resident_run<MD, STENCIL, I_EULER>(pb, rl, s);
+    case I_HEUN: return resident_run<MD, STENCIL, I_HEUN>(pb, rl, s);
+    case I_RK4: return resident_run<MD, STENCIL, I_RK4>(pb, rl, s);
+  }
+  return cudaErrorInvalidValue;
+}
+
+template <class MD>
+cudaError_t resident_by_stencil(const Problem& pb, const ResidentLaunch& rl, cudaStream_t s) {
+  switch (pb.stencil) {
+    case S_LAP5: return resident_by_integrator<MD, S_LAP5>(pb, rl, s);
+    case S_LAP9X4: return resident_by_integrator<MD, S_LAP9X4>(pb, rl, s);
+    case S_BOX9: return resident_by_integrator<MD, S_BOX9>(pb, rl, s);
+  }
+  return cudaErrorInvalidValue;
+}
+
+}  // namespace cardiac

@@ -56,7 +56,7 @@ CASES += [(BOCF, s, i) for s in (LAP5, LAP9X4, BOX9) for i in (RL, IE)]
 
 # CARDIAC_PLAN_* (+ parameter): STAGE with its DIRECT kernels, STAGE with the TMA-ring kernels
 # (forced: AUTO would pick DIRECT at these oracle-sized grids), FUSED
-STAGE, RING, FUSED = (1, 1), (1, 2), 2
+STAGE, RING, FUSED, PERSISTENT = (1, 1), (1, 2), 2, 3
 PLAN_CASES = [(m, s, i, STAGE) for (m, s, i) in CASES]
 PLAN_CASES += [(m, s, i, p) for (m, s, i) in CASES if i in (EULER, HEUN, RK4) for p in (RING, FUSED)]
 
@@ -74,6 +74,58 @@ def test_parity_one_and_hundred_steps(C, model, stencil, integ, plan):
     assert np.all(np.isfinite(got))
     assert maxabs(got, ref) <= TOL_100
     assert maxabs(got, Z) > 1e-6          # it did move
+
+
+# ----------------------------------------------------------------------------- plan PERSISTENT (grid resident on one SM)
+@pytest.mark.parametrize("model,stencil,integ", [(m, s, i) for m in (FHN, KARMA, BOCF) for s in (LAP5, LAP9X4, BOX9)
+                                                 for i in (EULER, HEUN, RK4)])
+def test_parity_persistent_plan(C, model, stencil, integ):
+    """One launch for all steps, one cluster per batch member: 47 x 40 (odd width: the padded half
+    pair; two CTAs of 20 rows exchanging ghost rows through distributed shared memory), batch 3;
+    against the oracle, against plan
+    FUSED to roundoff (same formulation; the compiler contracts the inlined reaction differently in
+    the two kernels) and bitwise against itself in chunks."""
+    cfg, Z = make(model, 47, 40, stencil, integ, batch=3)
+    got1 = gpu_run(C, cfg, Z, 1, plan=PERSISTENT)
+    assert maxabs(got1, O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 1)) <= TOL_1
+    got = gpu_run(C, cfg, Z, 100, plan=PERSISTENT)
+    ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 100)
+    assert maxabs(got, ref) <= TOL_100
+    assert maxabs(got, Z) > 1e-6
+    assert maxabs(got, gpu_run(C, cfg, Z, 100, plan=FUSED)) <= 1e-12
+    assert np.array_equal(got, gpu_run(C, cfg, Z, 100, plan=PERSISTENT, chunks=[1, 33, 66]))
+
+
+@pytest.mark.parametrize("model,stencil,nx,ny,bc", [(FHN, LAP9X4, 5, 5, 0), (KARMA, BOX9, 3, 3, 0), (FHN, LAP9X4, 64, 64, 1),
+                                                    (KARMA, LAP5, 33, 4, 1), (BOCF, LAP9X4, 64, 32, 0), (BOCF, BOX9, 37, 50, 1),
+                                                    (FHN, LAP9X4, 1000, 9, 0), (KARMA, BOX9, 176, 176, 1),
+                                                    (BOCF, LAP9X4, 128, 125, 0), (FHN, BOX9, 90, 61, 0)])
+def test_parity_persistent_edges(C, model, stencil, nx, ny, bc):
+    """Minimum sizes (one CTA), the periodic boundary across the cluster (the first slab reads the
+    last one), slabs of r rows with empty trailing CTAs (1000 x 9 over 8 CTAs), the capacity limits
+    (8 x 4096 / 8 x 2048 cells) and a ragged last slab (61 rows over 8 CTAs)."""
+    cfg, Z = make(model, nx, ny, stencil, RK4, boundary=bc)
+    got = gpu_run(C, cfg, Z, 30, plan=PERSISTENT)
+    ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 30)
+    assert maxabs(got, ref) <= TOL_100
+
+
+def test_persistent_plan_limits_and_auto(C):
+    cfg, _ = make(FHN, 200, 200, LAP5, RK4)                    # 40000 cells: more than 8 x 4096
+    with C.Context.from_config(cfg) as ctx:
+        assert ctx.plan == FUSED
+        with pytest.raises(C.CardiacError):
+            C.cardiac_set_plan(ctx.ctx, PERSISTENT, 0)
+    cfg, Z = make(FHN, 64, 64, LAP5, EULER)
+    with C.Context.from_config(cfg) as ctx:
+        assert ctx.plan == PERSISTENT                           # AUTO picks it for config-1-sized grids
+        ctx.set_state(Z); ctx.step(200)
+        assert ctx.launches == 1
+    cfg, _ = make(BOCF, 40, 40, LAP5, RL)
+    with C.Context.from_config(cfg) as ctx:
+        assert ctx.plan == 1
+        with pytest.raises(C.CardiacError):
+            C.cardiac_set_plan(ctx.ctx, PERSISTENT, 0)
 
 
 @pytest.mark.parametrize("model,stencil,integ", [(FHN, LAP9X4, RK4), (KARMA, LAP5, RK4), (BOCF, LAP9X4, RK4),

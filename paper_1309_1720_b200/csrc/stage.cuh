@@ -82,6 +82,7 @@ struct Stencil<S_BOX9> {
 
 // 128-bit accesses of an x-adjacent pair of cells ("vector width 2 for doubles")
 CARDIAC_D double2 ld2(const double* p) { return *reinterpret_cast<const double2*>(p); }
+CARDIAC_D void prefetch_l1(const double* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 CARDIAC_D void st2(double* p, double a, double b) { *reinterpret_cast<double2*>(p) = make_double2(a, b); }
 
 // integer-weight stencil sums of the two cells (x, x+1) of row `row`; interior, no boundary logic

@@ -98,6 +98,20 @@ __global__ void __launch_bounds__(TX* TY, 4)
   const bool interior = x0 >= 2 && x0 + 2 * TX + 2 <= nx && j0 >= R && j0 + TY + R <= ny;
   if (interior && KIND != K_RL && KIND != K_IE) {
     const int row = j * pitch, o = row + x;
+    // The gating fields are first used ~400 instructions into the reaction and y at its very end;
+    // under the 64-register cap ptxas sinks those loads next to their use (a second and third exposed
+    // latency per warp).  Asking L1 for the lines now costs no register; the late loads then hit.
+    // (Not for the 8 extra operand streams of K_RK4F: 4 blocks x 12 lines per thread overflow L1.)
+    if (KIND != K_RK4F) {
+      if (NV > 2) {   // only where the reaction is long enough to hide a DRAM latency (BOCF)
+#pragma unroll
+        for (int q = ND; q < NV; ++q) prefetch_l1(in + o + q * a.g.fstride);
+      }
+      if (KIND == K_BASE) {
+#pragma unroll
+        for (int q = 0; q < NV; ++q) prefetch_l1(yb + o + q * a.g.fstride);
+      }
+    }
     double2 zz[NV];
 #pragma unroll
     for (int q = 0; q < NV; ++q) zz[q] = ld2(in + o + q * a.g.fstride);

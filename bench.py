@@ -39,8 +39,33 @@ def algo_bytes_per_cell_step(cfg) -> int:
     return 8 * ALGO_DOUBLES[cfg.integrator] * cfg.n_v
 
 
+# Algorithmic FP64 work per cell-step of the five configs: FP64 instructions (DFMA + DMUL + DADD) and
+# flops (DFMA = 2) of the non-redundant update of ONE cell through all substeps, counted in the SASS of
+# the stage kernels (cuobjdump, body of ring_stage_kernel<model, stencil, kind>, per pair / 2; DESIGN.md
+# "Roofline").  Peak: 148 SM x 64 FP64 lanes/clk x 1.965 GHz = 18.6 T instr/s = 37.2 TFLOP/s.
+FP64_PER_CELL_STEP = {   # (model, stencil, integrator): (instructions, flops)
+    (W.FHN, W.LAP5, W.EULER): (18, 26),
+    (W.FHN, W.LAP9X4, W.RK4): (120, 170),
+    (W.KARMA, W.LAP5, W.RK4): (220, 342),
+    (W.BOCF, W.LAP9X4, W.RK4): (633, 1045),
+}
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+
+
 def floor_bytes_per_cell_step(cfg) -> int:
     return 16 * cfg.n_v   # read + write every field once, if all stages were fused on chip
+
+
+def fp64_view(cfg, gcell_steps_per_s):
+    """The other candidate bound of north_star: algorithmic FP64 flops per cell-step at the FP64 peak."""
+    k = (cfg.model, cfg.stencil, cfg.integrator)
+    if k not in FP64_PER_CELL_STEP:
+        return None
+    instr, flops = FP64_PER_CELL_STEP[k]
+    ach = gcell_steps_per_s * flops / 1e3
+    return {"achieved": ach, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach / FP64_PEAK_TFLOPS,
+            "flops_per_cell_step": flops, "fp64_instructions_per_cell_step": instr,
+            "peak_source": "derived: 148 SM x 64 FP64 lanes/clk x 2 x 1.965 GHz (DESIGN.md)"}
 
 
 def measured_peaks() -> tuple[float, str]:
@@ -204,6 +229,36 @@ def time_config(C, torch, cfg, Z0, steps, warmup, flush, plan=0, plan_param=0):
     return ms, launches, plan_used
 
 
+def run_sweep(args):
+    """Size sweep 'S' (the shape of the paper's Fig. 5): each model, RK4,
+    N = 64 .. 8192, AUTO plan and the STAGE plan; one JSON line.  Not the bench line."""
+    import torch
+    torch.cuda.set_device(0)
+    from paper_1309_1720_b200 import cardiac as C
+    peak, _ = measured_peaks()
+    rows = []
+    for model in (W.FHN, W.KARMA, W.BOCF):
+        for n in W.sweep_sizes():
+            cfg = W.sweep_config(model, n)
+            Z = W.sweep_state(cfg)
+            for plan in (0, 1):
+                with C.Context.from_config(cfg, plan=plan) as ctx:
+                    used = ctx.plan
+                    if plan == 1 and rows and rows[-1]["n"] == n and rows[-1]["plan"] == "stage":
+                        continue                              # AUTO already was STAGE
+                    ctx.set_state(Z)
+                    ctx.step(cfg.nsteps)
+                    torch.cuda.synchronize()
+                    best = min(C.cardiac_time_steps(ctx.ctx, cfg.nsteps, 1) for _ in range(3))
+                v = cfg.cells * cfg.nsteps / (best * 1e-3) / 1e9
+                rows.append({"model": W.MODEL_NAMES[model], "n": n, "stencil": W.STENCIL_NAMES[cfg.stencil],
+                             "plan": PLAN_NAMES.get(used, str(used)), "nsteps": cfg.nsteps,
+                             "us_per_step": best * 1e3 / cfg.nsteps, "value": v, "unit": UNIT,
+                             "hbm_frac_stage_sync": v * algo_bytes_per_cell_step(cfg) / peak})
+            del Z
+    print(json.dumps({"sweep": rows, "integrator": "rk4", "peak_gbs": peak}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -215,6 +270,7 @@ def main():
     ap.add_argument("--plan-param", type=int, default=0)
     ap.add_argument("--nsteps", type=int, default=0, help="override the config's time steps per run (profiling only)")
     ap.add_argument("--no-extras", action="store_true", help="skip cpu_baseline, e2e and the other configs")
+    ap.add_argument("--sweep", action="store_true", help="size sweep S of SURVEY.md 8(d) instead of the bench line")
     args = ap.parse_args()
     if args.warmup < 3 and not args.no_extras:
         args.warmup = 3                         # timing rule: W >= 3
@@ -227,6 +283,10 @@ def main():
 
     if args.impl == "reference":
         run_reference(args, cfg, rank)
+        return
+    if args.sweep:
+        if rank == 0:
+            run_sweep(args)
         return
 
     import torch
@@ -287,6 +347,7 @@ def main():
                 "floor_bytes_per_cell_step": floor_bytes_per_cell_step(cfg),
                 "frac_of_fused_floor": (floor_bytes_per_cell_step(cfg) * cfg.cells * cfg.nsteps * args.steps
                                         / (ms * 1e-3) / 1e9) / peak,
+                "fp64": fp64_view(cfg, value),
                 "note": ("state is L2-resident within a step for this config (working set "
                          f"{cfg.cells * cfg.n_v * 8 / 2**20:.0f} MiB per buffer set): frac > 1 is possible and "
                          "means less DRAM traffic than the stage-synchronous count")

@@ -118,7 +118,8 @@ int cardiac_set_stream(cardiac_ctx*, void* cuda_stream);
 
 /* Choose the execution plan (CARDIAC_PLAN_*).  CARDIAC_ERR_INVALID if the plan does not support
  * the context's (model, scheme, size). `param` is plan specific: FUSED + Euler = time steps per
- * launch (0 = default); STAGE = kernel implementation (0 = by size, 1 = DIRECT: every thread loads
+ * launch (0 = default); FUSED + Heun/RK4 = window (0 = by size, 1 = 80x48 cells, one CTA per SM,
+ * 2 = 48x40 cells, two CTAs per SM, two-field models only); STAGE = kernel implementation (0 = by size, 1 = DIRECT: every thread loads
  * its own operands, 2 = RING: persistent CTAs fed by a TMA shared-memory ring; same results
  * bitwise); otherwise 0. */
 int cardiac_set_plan(cardiac_ctx*, int plan, int param);

@@ -78,6 +78,20 @@ void carve(cardiac_ctx* c) {
 // round trip per substep dominates (FHN, Karma); the 4-field ionic model is FP64-pipe bound and its
 // register-resident patches are too small to amortise an 8-cell halo, so it stays stage-synchronous
 // (DESIGN.md "Plans").
+// FUSED + Heun/RK4: which window.  1 = large (80 x 48, one CTA per SM), 2 = small (48 x 40, two CTAs
+// per SM; two-field models).  Measured on B200: with a halo of H <= 4 cells the two
+// co-resident CTAs hide each other's load and barrier phases and the small window wins at every size
+// (Karma LAP5 RK4 2048^2: 30.9 -> 36.8 Gcell-step/s); with H = 8 its 40 % useful cells lose against
+// 53 % unless the whole grid is one wave of small tiles (<= 256^2: 7.7 -> 6.3 us per step).
+int fused_window_auto(const Problem& pb) {
+  if (pb.nv > 2 || pb.integrator == I_EULER) return 1;
+  const int H = pb.radius * stages_of(pb.integrator);
+  if (H <= 4) return 2;
+  const long long tw = 48 - 2 * H, th = 40 - 2 * H;
+  const long long ctas = ((pb.nx + tw - 1) / tw) * ((pb.ny + th - 1) / th) * pb.batch;
+  return ctas <= 148 ? 2 : 1;
+}
+
 int auto_plan(const Problem& pb) {
   const bool rk_like = pb.integrator == I_EULER || pb.integrator == I_HEUN || pb.integrator == I_RK4;
   // a grid that fits one SM never leaves it: the paper's launch-bound regime N < N0
@@ -86,9 +100,14 @@ int auto_plan(const Problem& pb) {
   return CARDIAC_PLAN_STAGE;
 }
 
+// FUSED + Heun/RK4: plan_param 1 = large window, 2 = small window (set_plan resolves 0)
+bool fused_small(const cardiac_ctx* c) {
+  return c->plan == CARDIAC_PLAN_FUSED && c->pb.integrator != I_EULER && c->plan_param == 2;
+}
+
 // Plan FUSED: one launch advances `ksteps` time steps (1, or kEulerBlock Euler steps), ping-pong.
 int enqueue_fused(cardiac_ctx* c, cudaStream_t s, int ksteps) {
-  TileLaunch tl{c->buf[c->cur], c->buf[1 - c->cur], ksteps};
+  TileLaunch tl{c->buf[c->cur], c->buf[1 - c->cur], ksteps, fused_small(c)};
   cudaError_t e = launch_fused(c->pb, tl, s);
   if (e != cudaSuccess) return fail_cuda(c, e, "fused launch");
   c->launches++;
@@ -279,7 +298,7 @@ cardiac_ctx* cardiac_create(int model, int nx, int ny, double dx, double dt, int
   c->nbuf = buffers_of(integ);
   c->plan_req = CARDIAC_PLAN_AUTO;
   c->plan = auto_plan(pb);
-  c->plan_param = (c->plan == CARDIAC_PLAN_FUSED && integ == I_EULER) ? kEulerBlock : 0;
+  c->plan_param = c->plan != CARDIAC_PLAN_FUSED ? 0 : (integ == I_EULER ? kEulerBlock : fused_window_auto(pb));
   e = cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking);
   if (e != cudaSuccess) {
     delete c;
@@ -331,8 +350,11 @@ int cardiac_set_plan(cardiac_ctx* c, int plan, int param) {
       rparam = param == 0 ? kEulerBlock : param;
       if (rparam != 1 && rparam != kEulerBlock)
         return fail(c, CARDIAC_ERR_INVALID, "FUSED + Euler: steps per launch must be 1 or 4");
-    } else if (param != 0) {
-      return fail(c, CARDIAC_ERR_INVALID, "plan parameter must be 0");
+    } else {
+      if (param < 0 || param > 2 || (param == 2 && c->pb.nv > 2))
+        return fail(c, CARDIAC_ERR_INVALID,
+                    "FUSED + Heun/RK4: parameter 0 (auto), 1 (80x48 window) or 2 (48x40 window, 2-field models)");
+      rparam = param == 0 ? fused_window_auto(c->pb) : param;
     }
   } else if (resolved == CARDIAC_PLAN_PERSISTENT) {
     if (!resident_supported(c->pb))

@@ -32,9 +32,10 @@ struct StepScheme {
   static constexpr bool RK = INTEG != I_EULER;
 };
 
-template <int NTX_, int NTY_, int PR_>
+template <int NTX_, int NTY_, int PR_, int MINB_ = 1>
 struct TileGeom {
   static constexpr int NTX = NTX_, NTY = NTY_, PR = PR_;
+  static constexpr int MINB = MINB_;  // CTAs per SM the register budget is held to
   static constexpr int NT = NTX * NTY;
   static constexpr int EW = 2 * NTX, EH = PR * NTY;  // loaded window
 };

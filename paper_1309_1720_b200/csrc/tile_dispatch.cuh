@@ -9,20 +9,31 @@ namespace cardiac {
 
 // window geometry per (model, halo): 2*NTX x PR*NTY cells, NTX*NTY threads, one CTA per SM.
 // The 4-field ionic model keeps 11 doubles per cell in registers, so its patches are smaller.
-template <class MD, int H>
+template <class MD, int H, bool SMALL>
 struct FusedGeom {
   using type = TileGeom<40, 12, 4>;  // 80 x 48 window, 480 threads
 };
-template <int VARIANT, int H>
-struct FusedGeom<Model<M_BOCF, VARIANT>, H> {
+// Mid-size grids (the paper's own range, 256^2 - 768^2) give the large window fewer
+// tiles than there are SMs, and a step then costs one CTA lifetime (~7.5 us) whatever the size: the
+// small window halves the cells per thread (2 x 2 instead of 2 x 4) and lets two CTAs share an SM.
+template <class MD, int H>
+struct FusedGeom<MD, H, true> {
+  using type = TileGeom<24, 20, 2, 2>;  // 48 x 40 window, 480 threads, 2 CTAs per SM
+};
+template <int VARIANT, int H, bool SMALL>
+struct FusedGeom<Model<M_BOCF, VARIANT>, H, SMALL> {
   using type = TileGeom<24, 16, 2>;  // 48 x 32 window, 384 threads
 };
 
 template <class MD, int STENCIL, int INTEG, int KSTEPS, class TG>
-__global__ void __launch_bounds__(TG::NT, 1)
+__global__ void __launch_bounds__(TG::NT, TG::MINB)
     fused_step_kernel(const __grid_constant__ TileArgs<MD> a) {
   using E = TileEngine<MD, STENCIL, INTEG, KSTEPS, TG>;
   extern __shared__ double2 smem_fused[];
+  // programmatic dependent launch: this grid may be scheduled while the previous time step's grid
+  // drains; every global access below waits for that grid to complete and flush
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const long long base = (long long)blockIdx.z * a.g.bstride;
   E::run(a, a.in + base, a.out + base, blockIdx.x, blockIdx.y, reinterpret_cast<double*>(smem_fused));
 }
@@ -48,10 +59,10 @@ void fill_tile_args(const Problem& pb, int stencil, TileArgs<MD>& a) {
   a.nsteps = 0; a.tiles_x = a.tiles_y = 0; a.step_base = 0;
 }
 
-template <class MD, int STENCIL, int INTEG, int KSTEPS>
+template <class MD, int STENCIL, int INTEG, int KSTEPS, bool SMALL = false>
 cudaError_t fused_run(const Problem& pb, const TileLaunch& tl, cudaStream_t stream) {
   constexpr int H = stencil_radius(STENCIL) * StepScheme<INTEG, KSTEPS>::NS;
-  using TG = typename FusedGeom<MD, H>::type;
+  using TG = typename FusedGeom<MD, H, SMALL>::type;
   using E = TileEngine<MD, STENCIL, INTEG, KSTEPS, TG>;
   auto kern = fused_step_kernel<MD, STENCIL, INTEG, KSTEPS, TG>;
   static bool configured = false;  // per instantiation
@@ -64,15 +75,30 @@ cudaError_t fused_run(const Problem& pb, const TileLaunch& tl, cudaStream_t stre
   fill_tile_args<MD>(pb, STENCIL, a);
   a.in = tl.in; a.out = tl.out;
   dim3 grid((pb.nx + E::TW - 1) / E::TW, (pb.ny + E::TH - 1) / E::TH, pb.batch);
-  kern<<<grid, TG::NT, E::SMEM_BYTES, stream>>>(a);
-  return cudaGetLastError();
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = dim3(TG::NT);
+  cfg.dynamicSmemBytes = E::SMEM_BYTES;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, a);
 }
 
 template <class MD, int STENCIL>
 cudaError_t fused_by_integrator(const Problem& pb, const TileLaunch& tl, cudaStream_t s) {
   switch (pb.integrator) {
-    case I_RK4: return fused_run<MD, STENCIL, I_RK4, 1>(pb, tl, s);
-    case I_HEUN: return fused_run<MD, STENCIL, I_HEUN, 1>(pb, tl, s);
+    case I_RK4:
+      if constexpr (MD::NV <= 2)
+        if (tl.small) return fused_run<MD, STENCIL, I_RK4, 1, true>(pb, tl, s);
+      return fused_run<MD, STENCIL, I_RK4, 1>(pb, tl, s);
+    case I_HEUN:
+      if constexpr (MD::NV <= 2)
+        if (tl.small) return fused_run<MD, STENCIL, I_HEUN, 1, true>(pb, tl, s);
+      return fused_run<MD, STENCIL, I_HEUN, 1>(pb, tl, s);
     case I_EULER:
       if (tl.ksteps == 1) return fused_run<MD, STENCIL, I_EULER, 1>(pb, tl, s);
       if (tl.ksteps == kEulerBlock) return fused_run<MD, STENCIL, I_EULER, kEulerBlock>(pb, tl, s);

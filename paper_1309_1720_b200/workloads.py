@@ -256,6 +256,30 @@ def synthetic_base_cfg5(cfg: Config) -> np.ndarray:
     return z
 
 
+def sweep_sizes() -> list[int]:
+    """Grid sizes of the size sweep 'S' of SURVEY.md §8(d): the paper's Fig. 5 sweep through
+    N0 ~ 362 extended to streaming sizes."""
+    return [64, 128, 256, 362, 512, 768, 1024, 2048, 4096, 8192]
+
+
+def sweep_config(model: int, n: int, stencil: int | None = None, integrator: int = RK4) -> Config:
+    if stencil is None:
+        stencil = LAP5 if model == KARMA else LAP9X4          # the stencils of configs 2-4
+    nsteps = max(8, min(200, (1 << 28) // (n * n) * 8))       # 200 steps up to 1024^2, fewer beyond
+    return make_config(f"sweep{n}", model, n, stencil, integrator, nsteps, seed=9)
+
+
+def sweep_state(cfg: Config, base: int = 256) -> np.ndarray:
+    """Config-3-style block-noise state of a base x base grid, repeated
+    periodically to cfg.nx x cfg.ny: generating 8192^2 x 4 fields block by block on the host would
+    take longer than the measurement; the kernels' speed does not depend on the values."""
+    b = min(base, cfg.nx, cfg.ny)
+    small = state_blocks(replace(cfg, nx=b, ny=b, batch=1))
+    ry, rx = -(-cfg.ny // b), -(-cfg.nx // b)
+    z = np.tile(small, (cfg.batch, 1, ry, rx))[:, :, :cfg.ny, :cfg.nx]
+    return np.ascontiguousarray(z)
+
+
 def initial_state(cfg: Config) -> np.ndarray:
     """Initial state of a (possibly scaled) baseline config, dense [batch][n_v][ny][nx]."""
     base = cfg.name.split("@")[0]

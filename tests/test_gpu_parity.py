@@ -76,6 +76,25 @@ def test_parity_one_and_hundred_steps(C, model, stencil, integ, plan):
     assert maxabs(got, Z) > 1e-6          # it did move
 
 
+# ----------------------------------------------------------------------------- plan FUSED, both windows
+@pytest.mark.parametrize("model,stencil,integ", [(m, s, i) for m in (FHN, KARMA) for s in (LAP5, LAP9X4, BOX9)
+                                                 for i in (HEUN, RK4)])
+def test_parity_fused_small_window(C, model, stencil, integ):
+    """The 48 x 40 window (two CTAs per SM) on a grid of several ragged tiles, against the oracle and
+    against the 80 x 48 window; AUTO resolves to one of the two."""
+    cfg, Z = make(model, 150, 97, stencil, integ, seed=5)
+    small = gpu_run(C, cfg, Z, 40, plan=(2, 2))
+    ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 40)
+    assert maxabs(small, ref) <= TOL_100
+    large = gpu_run(C, cfg, Z, 40, plan=(2, 1))
+    assert maxabs(small, large) <= 1e-12
+    auto = gpu_run(C, cfg, Z, 40, plan=(2, 0))
+    assert np.array_equal(auto, small) or np.array_equal(auto, large)
+    with C.Context.from_config(W.make_config("b", BOCF, 64, LAP5, RK4, 0), plan=2) as ctx:
+        with pytest.raises(C.CardiacError):
+            C.cardiac_set_plan(ctx.ctx, 2, 2)          # the 4-field model has one window only
+
+
 # ----------------------------------------------------------------------------- plan PERSISTENT (grid resident on one SM)
 @pytest.mark.parametrize("model,stencil,integ", [(m, s, i) for m in (FHN, KARMA, BOCF) for s in (LAP5, LAP9X4, BOX9)
                                                  for i in (EULER, HEUN, RK4)])

@@ -266,22 +266,67 @@ int oracle_laplacian(const double* U, double* L, int nx, int ny, double dx, int 
   return 0;
 }
 
+/* 3-D ("three-dimensional simulations (corresponding to ventricular tissue)"; DESIGN.md f4):
+ * L = lap(U) on an nz x ny x nx grid (x fastest), spacing dx = dy = dz, the same per-axis weights
+ * as in 2-D applied along x, y and z — S_LAP5 becomes the 7-point stencil, S_LAP9X4 the 13-point
+ * 4th-order cross; Eq. 6's 3 x 3 box (S_BOX9) has no 3-D counterpart in the paper: rejected.
+ * Same index reflection / wrap per axis, same difference form. */
+int oracle_laplacian3d(const double* U, double* L, int nx, int ny, int nz, double dx, int stencil,
+                       int boundary) {
+  int r = (stencil == S_LAP9X4) ? 2 : 1;
+  if ((stencil != S_LAP5 && stencil != S_LAP9X4) || nx < 2 * r + 1 || ny < 2 * r + 1 || nz < 2 * r + 1)
+    return -1;
+  double h2 = dx * dx;
+#ifdef _OPENMP
+#pragma omp parallel for
+#endif
+  for (int k = 0; k < nz; ++k) {
+    for (int j = 0; j < ny; ++j) {
+      for (int i = 0; i < nx; ++i) {
+#define UU(di, dj, dk)                                                                   \
+  U[((size_t)bidx(k + (dk), nz, boundary) * ny + bidx(j + (dj), ny, boundary)) * nx + \
+    bidx(i + (di), nx, boundary)]
+        double u0 = U[((size_t)k * ny + j) * nx + i];
+        double s;
+        if (stencil == S_LAP5) {
+          double ax = (UU(1, 0, 0) - u0) + (UU(-1, 0, 0) - u0);
+          double ay = (UU(0, 1, 0) - u0) + (UU(0, -1, 0) - u0);
+          double az = (UU(0, 0, 1) - u0) + (UU(0, 0, -1) - u0);
+          s = (ax + ay) + az;
+        } else {
+          double c1 = 4.0 / 3.0, c2 = -1.0 / 12.0;
+          double ax = c1 * ((UU(1, 0, 0) - u0) + (UU(-1, 0, 0) - u0)) + c2 * ((UU(2, 0, 0) - u0) + (UU(-2, 0, 0) - u0));
+          double ay = c1 * ((UU(0, 1, 0) - u0) + (UU(0, -1, 0) - u0)) + c2 * ((UU(0, 2, 0) - u0) + (UU(0, -2, 0) - u0));
+          double az = c1 * ((UU(0, 0, 1) - u0) + (UU(0, 0, -1) - u0)) + c2 * ((UU(0, 0, 2) - u0) + (UU(0, 0, -2) - u0));
+          s = (ax + ay) + az;
+        }
+#undef UU
+        L[((size_t)k * ny + j) * nx + i] = s / h2;
+      }
+    }
+  }
+  return 0;
+}
+
 /* ------------------------------------------------------------------ right-hand side */
 
 typedef struct {
   int model, stencil, integrator, boundary, variant;
-  int nx, ny, nv, nd;
+  int nx, ny, nz, nv, nd;   /* nz == 1: the 2-D problem of the paper */
   double dx, dt;
   const double* p;
 } problem;
 
-/* F = D lap(Z) + N[Z] for one state Z[n_v][ny][nx]; lapbuf is scratch of ny*nx doubles.
+/* F = D lap(Z) + N[Z] for one state Z[n_v][nz][ny][nx]; lapbuf is scratch of nz*ny*nx doubles.
  * Order as in PAPER.md:132: non-local terms first, then the local terms, then combined. */
 static void rhs(const problem* q, const double* Z, double* F, double* lapbuf) {
-  size_t n = (size_t)q->nx * q->ny;
+  size_t n = (size_t)q->nx * q->ny * q->nz;
   for (int f = 0; f < q->nd; ++f) {
     double D = (q->model == M_FHN) ? q->p[f] : q->p[0];
-    oracle_laplacian(Z + f * n, lapbuf, q->nx, q->ny, q->dx, q->stencil, q->boundary);
+    if (q->nz > 1)
+      oracle_laplacian3d(Z + f * n, lapbuf, q->nx, q->ny, q->nz, q->dx, q->stencil, q->boundary);
+    else
+      oracle_laplacian(Z + f * n, lapbuf, q->nx, q->ny, q->dx, q->stencil, q->boundary);
 #ifdef _OPENMP
 #pragma omp parallel for
 #endif
@@ -306,7 +351,7 @@ int oracle_rhs(int model, int nx, int ny, double dx, int scheme, const double* p
   problem q;
   q.model = model; q.stencil = scheme & 0xff; q.integrator = (scheme >> 8) & 0xff;
   q.boundary = (scheme >> 16) & 0xff; q.variant = (scheme >> 24) & 0xff;
-  q.nx = nx; q.ny = ny; q.dx = dx; q.dt = 0.0;
+  q.nx = nx; q.ny = ny; q.nz = 1; q.dx = dx; q.dt = 0.0;
   q.nv = oracle_num_fields(model);
   if (q.nv < 0) return -1;
   q.nd = num_diffusing(model);
@@ -322,7 +367,7 @@ int oracle_rhs(int model, int nx, int ny, double dx, int scheme, const double* p
 
 /* One time step of one state, in place.  w = workspace of 5*n_v*n + n doubles. */
 static void step_once(const problem* q, double* Z, double* w) {
-  size_t n = (size_t)q->nx * q->ny, N = n * q->nv;
+  size_t n = (size_t)q->nx * q->ny * q->nz, N = n * q->nv;
   double dt = q->dt;
   double *K1 = w, *K2 = w + N, *K3 = w + 2 * N, *K4 = w + 3 * N, *Y = w + 4 * N, *lapbuf = w + 5 * N;
 
@@ -378,16 +423,16 @@ static void step_once(const problem* q, double* Z, double* w) {
   }
 }
 
-/* Advance `batch` independent states Z[batch][n_v][ny][nx] by nsteps steps, in place.
- * params == NULL: the default block.  Returns 0, or -1 on invalid arguments, -2 on allocation
- * failure. */
-int oracle_step(int model, int nx, int ny, double dx, double dt, int scheme, int batch,
-                const double* params, double* Z, long long nsteps) {
+/* Advance `batch` independent states Z[batch][n_v][nz][ny][nx] by nsteps steps, in place (nz == 1:
+ * the 2-D problem).  params == NULL: the default block.  Returns 0, or -1 on invalid arguments,
+ * -2 on allocation failure. */
+int oracle_step3d(int model, int nx, int ny, int nz, double dx, double dt, int scheme, int batch,
+                  const double* params, double* Z, long long nsteps) {
   double pdef[32];
   problem q;
   q.model = model; q.stencil = scheme & 0xff; q.integrator = (scheme >> 8) & 0xff;
   q.boundary = (scheme >> 16) & 0xff; q.variant = (scheme >> 24) & 0xff;
-  q.nx = nx; q.ny = ny; q.dx = dx; q.dt = dt;
+  q.nx = nx; q.ny = ny; q.nz = nz; q.dx = dx; q.dt = dt;
   q.nv = oracle_num_fields(model);
   if (q.nv < 0) return -1;
   q.nd = num_diffusing(model);
@@ -396,16 +441,22 @@ int oracle_step(int model, int nx, int ny, double dx, double dt, int scheme, int
       q.variant > V_TANHFREE) return -1;
   if (q.integrator >= I_RUSH_LARSEN && model != M_BOCF) return -1;
   if (nx < 2 * r + 1 || ny < 2 * r + 1 || batch < 1 || nsteps < 0) return -1;
+  if (nz != 1 && (nz < 2 * r + 1 || q.stencil == S_BOX9)) return -1;
   if (!(dx > 0.0) || !(dt > 0.0) || !isfinite(dx) || !isfinite(dt)) return -1;
   if (params) q.p = params; else { oracle_default_params(model, pdef); q.p = pdef; }
 
-  size_t n = (size_t)nx * ny, N = n * q.nv;
+  size_t n = (size_t)nx * ny * nz, N = n * q.nv;
   double* w = (double*)malloc(sizeof(double) * (5 * N + n));
   if (!w) return -2;
   for (int b = 0; b < batch; ++b)
     for (long long s = 0; s < nsteps; ++s) step_once(&q, Z + (size_t)b * N, w);
   free(w);
   return 0;
+}
+
+int oracle_step(int model, int nx, int ny, double dx, double dt, int scheme, int batch,
+                const double* params, double* Z, long long nsteps) {
+  return oracle_step3d(model, nx, ny, 1, dx, dt, scheme, batch, params, Z, nsteps);
 }
 
 /* Finite-difference Jacobian-vector products of the flow map:

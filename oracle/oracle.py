@@ -43,6 +43,11 @@ def lib(omp: bool = False) -> ctypes.CDLL:
         L.oracle_step.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double,
                                   ctypes.c_double, ctypes.c_int, ctypes.c_int, _dp, _dp,
                                   ctypes.c_longlong]
+        L.oracle_laplacian3d.argtypes = [_dp, _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double,
+                                         ctypes.c_int, ctypes.c_int]
+        L.oracle_step3d.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double,
+                                    ctypes.c_double, ctypes.c_int, ctypes.c_int, _dp, _dp,
+                                    ctypes.c_longlong]
         L.oracle_jvp.argtypes = [_dp, ctypes.c_int, ctypes.c_size_t, ctypes.c_double, _dp]
         _loaded[omp] = L
     return _loaded[omp]
@@ -104,6 +109,35 @@ def laplacian(U, dx: float, stencil: int, boundary: int = 0) -> np.ndarray:
     if rc:
         raise ValueError("oracle_laplacian: invalid arguments")
     return L
+
+
+def laplacian3d(U, dx: float, stencil: int, boundary: int = 0) -> np.ndarray:
+    """3-D Laplacian of U[nz][ny][nx] (7-point for stencil 0, 13-point 4th-order cross for stencil 1)."""
+    U = _c(U)
+    nz, ny, nx = U.shape
+    L = np.empty_like(U)
+    rc = lib().oracle_laplacian3d(_ptr(U), _ptr(L), nx, ny, nz, float(dx), stencil, boundary)
+    if rc:
+        raise ValueError("oracle_laplacian3d: invalid arguments")
+    return L
+
+
+def step3d(model: int, Z, dx: float, dt: float, scheme: int, nsteps: int, params=None,
+           omp: bool = False) -> np.ndarray:
+    """Advance Z ([batch][n_v][nz][ny][nx] or [n_v][nz][ny][nx]) by nsteps; returns a new array."""
+    Z = np.array(Z, dtype=np.float64, order="C", copy=True)
+    shape = Z.shape
+    if Z.ndim == 4:
+        Z = Z[None]
+    batch, nv, nz, ny, nx = Z.shape
+    if nv != num_fields(model):
+        raise ValueError("wrong number of fields")
+    p = None if params is None else _c(params)
+    rc = lib(omp).oracle_step3d(model, nx, ny, nz, float(dx), float(dt), scheme, batch,
+                                None if p is None else _ptr(p), _ptr(Z), int(nsteps))
+    if rc:
+        raise ValueError(f"oracle_step3d failed ({rc})")
+    return Z.reshape(shape)
 
 
 def rhs(model: int, Z, dx: float, scheme: int, params=None) -> np.ndarray:

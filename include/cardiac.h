@@ -105,6 +105,14 @@ int cardiac_default_params(int model, double* p, int n);
  * The current CUDA device is captured.  Returns NULL on failure (text: cardiac_last_error(NULL)). */
 cardiac_ctx* cardiac_create(int model, int nx, int ny, double dx, double dt, int scheme, int batch);
 
+/* 3-D variant ("three-dimensional simulations (corresponding to ventricular tissue)";
+ * DESIGN.md f4): nz planes of ny x nx cells, spacing dx in all three directions; the stencil bits
+ * select the same per-axis weights applied along x, y and z (CARDIAC_LAP5 -> 7-point, CARDIAC_LAP9X4
+ * -> 13-point 4th-order cross; CARDIAC_BOX9 is 2-D only), the boundary rule applies per axis.  State
+ * layout: dense [batch][n_v][nz][ny][nx].  nz == 1 is cardiac_create(); otherwise nz >= 2r+1 and
+ * batch * nz <= 65535.  3-D contexts run plan STAGE. */
+cardiac_ctx* cardiac_create3d(int model, int nx, int ny, int nz, double dx, double dt, int scheme, int batch);
+
 /* Replace the model parameters (host array, n == cardiac_num_params(model)).  Takes effect for
  * subsequent steps.  M (Karma) must be an integer in [1, 16]. */
 int cardiac_set_params(cardiac_ctx*, const double* p, int n);

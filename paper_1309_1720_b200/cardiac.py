@@ -55,6 +55,7 @@ _sig = {
     "cardiac_num_params": (_i, [_i]),
     "cardiac_default_params": (_i, [_i, _dp, _i]),
     "cardiac_create": (_vp, [_i, _i, _i, _d, _d, _i, _i]),
+    "cardiac_create3d": (_vp, [_i, _i, _i, _i, _d, _d, _i, _i]),
     "cardiac_set_params": (_i, [_vp, _dp, _i]),
     "cardiac_get_params": (_i, [_vp, _dp, _i]),
     "cardiac_set_stream": (_i, [_vp, _vp]),
@@ -118,6 +119,13 @@ def cardiac_default_params(model: int) -> np.ndarray:
 
 def cardiac_create(model: int, nx: int, ny: int, dx: float, dt: float, scheme: int, batch: int = 1):
     ctx = _lib.cardiac_create(model, nx, ny, dx, dt, scheme, batch)
+    if not ctx:
+        raise CardiacError(CARDIAC_ERR_INVALID, (_lib.cardiac_last_error(None) or b"").decode())
+    return ctx
+
+
+def cardiac_create3d(model: int, nx: int, ny: int, nz: int, dx: float, dt: float, scheme: int, batch: int = 1):
+    ctx = _lib.cardiac_create3d(model, nx, ny, nz, dx, dt, scheme, batch)
     if not ctx:
         raise CardiacError(CARDIAC_ERR_INVALID, (_lib.cardiac_last_error(None) or b"").decode())
     return ctx
@@ -204,9 +212,11 @@ class Context:
     """RAII holder of a cardiac_ctx; torch provides the workspace memory and the stream."""
 
     def __init__(self, model, nx, ny, dx, dt, scheme, batch=1, plan=CARDIAC_PLAN_AUTO, plan_param=0,
-                 params=None, use_torch_memory=True):
-        self.shape = (batch, cardiac_num_fields(model), ny, nx)
-        self.ctx = cardiac_create(model, nx, ny, dx, dt, scheme, batch)
+                 params=None, use_torch_memory=True, nz=1):
+        nv = cardiac_num_fields(model)
+        self.shape = (batch, nv, ny, nx) if nz == 1 else (batch, nv, nz, ny, nx)
+        self.ctx = (cardiac_create(model, nx, ny, dx, dt, scheme, batch) if nz == 1 else
+                    cardiac_create3d(model, nx, ny, nz, dx, dt, scheme, batch))
         self._ws = None
         try:
             if params is not None:
@@ -227,7 +237,7 @@ class Context:
 
     @classmethod
     def from_config(cls, cfg, **kw):
-        return cls(cfg.model, cfg.nx, cfg.ny, cfg.dx, cfg.dt, cfg.scheme, cfg.batch, **kw)
+        return cls(cfg.model, cfg.nx, cfg.ny, cfg.dx, cfg.dt, cfg.scheme, cfg.batch, nz=getattr(cfg, "nz", 1), **kw)
 
     def set_state(self, src):
         cardiac_set_state(self.ctx, src)

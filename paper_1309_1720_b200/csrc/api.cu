@@ -95,6 +95,7 @@ int fused_window_auto(const Problem& pb) {
 int auto_plan(const Problem& pb) {
   const bool rk_like = pb.integrator == I_EULER || pb.integrator == I_HEUN || pb.integrator == I_RK4;
   // a grid that fits one SM never leaves it: the paper's launch-bound regime N < N0
+  if (pb.nz > 1) return CARDIAC_PLAN_STAGE;   // 3-D: the stage-synchronous plan only
   if (resident_preferred(pb)) return CARDIAC_PLAN_PERSISTENT;
   if (rk_like && pb.model != CARDIAC_BOCF) return CARDIAC_PLAN_FUSED;
   return CARDIAC_PLAN_STAGE;
@@ -250,7 +251,7 @@ int cardiac_default_params(int model, double* p, int n) {
   return CARDIAC_OK;
 }
 
-cardiac_ctx* cardiac_create(int model, int nx, int ny, double dx, double dt, int scheme, int batch) {
+cardiac_ctx* cardiac_create3d(int model, int nx, int ny, int nz, double dx, double dt, int scheme, int batch) {
   auto bad = [](const std::string& m) -> cardiac_ctx* { g_create_error = m; return nullptr; };
   g_create_error.clear();
   const int nv = cardiac_num_fields(model);
@@ -266,8 +267,13 @@ cardiac_ctx* cardiac_create(int model, int nx, int ny, double dx, double dt, int
   const int r = stencil_radius(stencil);
   if (nx < 2 * r + 1 || ny < 2 * r + 1) return bad("nx, ny must be >= 2*radius+1");
   if (nx > (1 << 20) || ny > (1 << 20) || (long long)((nx + 15) / 16 * 16) * ny >= (1LL << 31))
-    return bad("grid too large (a field must have fewer than 2^31 elements)");
+    return bad("grid too large (a plane must have fewer than 2^31 elements)");
   if (batch < 1 || batch > 65535) return bad("batch must be in [1, 65535]");
+  if (nz != 1) {   // 3-D: the same per-axis stencil along z
+    if (nz < 2 * r + 1) return bad("nz must be 1 (2-D) or >= 2*radius+1");
+    if (stencil == S_BOX9) return bad("the 3x3 box stencil (Eq. 6) is defined in 2-D only");
+    if ((long long)batch * nz > 65535) return bad("batch * nz must be <= 65535");
+  }
   if (!(dx > 0.0) || !std::isfinite(dx)) return bad("dx must be finite and > 0");
   if (!(dt > 0.0) || !std::isfinite(dt)) return bad("dt must be finite and > 0");
 
@@ -285,10 +291,11 @@ cardiac_ctx* cardiac_create(int model, int nx, int ny, double dx, double dt, int
   if (!c) return bad("out of host memory");
   Problem& pb = c->pb;
   pb.model = model; pb.stencil = stencil; pb.integrator = integ; pb.boundary = bc;
-  pb.variant = variant; pb.nx = nx; pb.ny = ny; pb.batch = batch; pb.nv = nv;
+  pb.variant = variant; pb.nx = nx; pb.ny = ny; pb.nz = nz; pb.batch = batch; pb.nv = nv;
   pb.nd = model == CARDIAC_FHN ? 2 : 1; pb.radius = r;
   pb.pitch = (nx + 15) / 16 * 16;
-  pb.fstride = (long long)pb.pitch * ny;
+  pb.zstride = pb.pitch * ny;
+  pb.fstride = (long long)pb.zstride * nz;
   pb.bstride = pb.fstride * nv;
   pb.dx = dx; pb.dt = dt;
   c->scheme = scheme;
@@ -305,6 +312,10 @@ cardiac_ctx* cardiac_create(int model, int nx, int ny, double dx, double dt, int
     return bad(std::string("cudaStreamCreate: ") + cudaGetErrorString(e));
   }
   return c;
+}
+
+cardiac_ctx* cardiac_create(int model, int nx, int ny, double dx, double dt, int scheme, int batch) {
+  return cardiac_create3d(model, nx, ny, 1, dx, dt, scheme, batch);
 }
 
 int cardiac_set_params(cardiac_ctx* c, const double* p, int n) {
@@ -343,7 +354,10 @@ int cardiac_set_plan(cardiac_ctx* c, int plan, int param) {
   if (resolved == CARDIAC_PLAN_STAGE) {
     if (param < 0 || param > 2)
       return fail(c, CARDIAC_ERR_INVALID, "STAGE: parameter must be 0 (auto), 1 (direct) or 2 (TMA ring)");
+    if (param == 2 && c->pb.nz > 1) return fail(c, CARDIAC_ERR_INVALID, "the TMA-ring stage kernels are 2-D only");
     rparam = param;
+  } else if (c->pb.nz > 1) {
+    return fail(c, CARDIAC_ERR_INVALID, "3-D contexts run plan STAGE only");
   } else if (resolved == CARDIAC_PLAN_FUSED) {
     if (!rk_like) return fail(c, CARDIAC_ERR_INVALID, "FUSED supports Euler, Heun and RK4 only");
     if (integ == I_EULER) {
@@ -402,7 +416,7 @@ int cardiac_set_state(cardiac_ctx* c, const double* src, int src_on_device) {
   c->cur = 0;
   CK(cudaMemcpy2DAsync(c->buf[0], (size_t)pb.pitch * sizeof(double), src,
                        (size_t)pb.nx * sizeof(double), (size_t)pb.nx * sizeof(double),
-                       (size_t)pb.ny * pb.nv * pb.batch,
+                       (size_t)pb.ny * pb.nz * pb.nv * pb.batch,
                        src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
   if (!src_on_device) CK(cudaStreamSynchronize(c->stream));
   c->has_state = true;
@@ -417,7 +431,7 @@ int cardiac_get_state(cardiac_ctx* c, double* dst, int dst_on_device) {
   const Problem& pb = c->pb;
   CK(cudaMemcpy2DAsync(dst, (size_t)pb.nx * sizeof(double), c->buf[c->cur],
                        (size_t)pb.pitch * sizeof(double), (size_t)pb.nx * sizeof(double),
-                       (size_t)pb.ny * pb.nv * pb.batch,
+                       (size_t)pb.ny * pb.nz * pb.nv * pb.batch,
                        dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
   if (!dst_on_device) CK(cudaStreamSynchronize(c->stream));
   return CARDIAC_OK;
@@ -479,7 +493,7 @@ int cardiac_get_jvp(cardiac_ctx* c, double eps, double* dst, int dst_on_device) 
     c->launches++;
     return CARDIAC_OK;
   }
-  size_t bytes = (size_t)pb.nx * pb.ny * pb.nv * (pb.batch - 1) * sizeof(double);
+  size_t bytes = (size_t)pb.nx * pb.ny * pb.nz * pb.nv * (pb.batch - 1) * sizeof(double);
   double* tmp = nullptr;
   CK(cudaMalloc(&tmp, bytes));
   cudaError_t e = launch_jvp(pb, c->buf[c->cur], eps, tmp, c->stream);

@@ -7,9 +7,10 @@ namespace cardiac {
 
 struct Problem {
   int model, stencil, integrator, boundary, variant;
-  int nx, ny, batch, nv, nd, radius;
+  int nx, ny, nz, batch, nv, nd, radius;   // nz == 1: 2-D
   int pitch;            // doubles per row
-  long long fstride;    // doubles per field
+  int zstride;          // doubles per plane (pitch * ny)
+  long long fstride;    // doubles per field (zstride * nz)
   long long bstride;    // doubles per batch member
   double dx, dt;
   double params[32];    // public parameter block (include/cardiac.h)
@@ -72,7 +73,7 @@ struct ResidentShape {
 };
 inline ResidentShape resident_shape(const Problem& pb) {
   ResidentShape rs{0, 0, 0};
-  if (pb.integrator > 2) return rs;  // Euler, Heun, RK4
+  if (pb.integrator > 2 || pb.nz > 1) return rs;  // Euler, Heun, RK4; 2-D
   const long long npx = (pb.nx + 1) / 2, cap = 512LL * (pb.nv > 2 ? 2 : 4);
   const size_t sp = 2 * (size_t)npx + 4;
   for (int c = 1; c <= 8; c *= 2) {

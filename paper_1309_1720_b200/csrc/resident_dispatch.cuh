@@ -21,6 +21,7 @@ cudaError_t resident_run(const Problem& pb, const ResidentLaunch& rl, cudaStream
   ResidentArgs<MD> a;
   a.in = rl.state; a.out = rl.state;
   a.g.nx = pb.nx; a.g.ny = pb.ny; a.g.pitch = pb.pitch; a.g.boundary = pb.boundary;
+  a.g.nz = 1; a.g.zstride = pb.zstride;
   a.g.fstride = pb.fstride; a.g.bstride = pb.bstride;
   a.nsteps = rl.nsteps;
   const ResidentShape rs = resident_shape(pb);

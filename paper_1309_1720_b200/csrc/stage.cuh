@@ -27,8 +27,10 @@ __host__ __device__ constexpr double stencil_norm(int stencil) {
 // row starts 128-byte aligned); x fastest.
 struct Geom {
   int nx, ny, pitch, boundary;
-  long long fstride;  // doubles between fields  (= pitch * ny)
+  long long fstride;  // doubles between fields  (= pitch * ny * nz)
   long long bstride;  // doubles between batch members (= fstride * n_v)
+  int nz;             // 1: the paper's 2-D problem; > 1: 3-D, planes of pitch * ny doubles
+  int zstride;        // doubles between planes (= pitch * ny)
 };
 
 template <class MD>
@@ -109,6 +111,21 @@ CARDIAC_D void stencil_pair(const double* __restrict__ U, int row, int x, int pi
     s1 = Stencil<S_BOX9>::apply(c.y, c.x, e, s.y, n.y, s.x, se, n.x, ne);
   }
 }
+
+// 3-D: what the z axis adds to the integer-weight sum of the 2-D stencil of the same family
+// (7-point = LAP5 + z arm, 13-point = LAP9X4 + z arm; same per-axis weights, DESIGN.md f4)
+template <int STENCIL>
+struct StencilZ;
+template <>
+struct StencilZ<S_LAP5> {
+  CARDIAC_D static double apply(double c, double d1, double u1) { return fma(-2.0, c, d1 + u1); }
+};
+template <>
+struct StencilZ<S_LAP9X4> {
+  CARDIAC_D static double apply(double c, double d1, double u1, double d2, double u2) {
+    return fma(-30.0, c, fma(16.0, d1 + u1, -(d2 + u2)));
+  }
+};
 
 // the RK combination of one field value, shared by every plan
 template <int KIND>

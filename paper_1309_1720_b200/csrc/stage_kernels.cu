@@ -21,6 +21,10 @@ namespace {
 
 constexpr int TX = 32, TY = 8;   // threads; the tile is 2*TX x TY cells
 
+// offsets inside a field: a 2-D field has fewer than 2^31 elements (checked at create), a 3-D one may not
+template <bool D3> struct Off { typedef int type; };
+template <> struct Off<true> { typedef long long type; };
+
 // one cell with the boundary rule applied per axis (Q3)
 template <int STENCIL>
 CARDIAC_D double stencil_edge(const double* __restrict__ U, int i, int j, int nx, int ny, int pitch,
@@ -41,11 +45,37 @@ CARDIAC_D double stencil_edge(const double* __restrict__ U, int i, int j, int nx
   }
 }
 
+// 3-D: the z arm of the pair (x, x+1) at offset o of a field, planes kz +- m inside the grid
+template <int STENCIL>
+CARDIAC_D void zarm_pair(const double* __restrict__ U, long long o, int zs, double2 c, double& s0, double& s1) {
+  const double2 d1 = ld2(U + o - zs), u1 = ld2(U + o + zs);
+  if (STENCIL == S_LAP9X4) {
+    const double2 d2 = ld2(U + o - 2 * (long long)zs), u2 = ld2(U + o + 2 * (long long)zs);
+    s0 += StencilZ<S_LAP9X4>::apply(c.x, d1.x, u1.x, d2.x, u2.x);
+    s1 += StencilZ<S_LAP9X4>::apply(c.y, d1.y, u1.y, d2.y, u2.y);
+  } else if (STENCIL == S_LAP5) {
+    s0 += StencilZ<S_LAP5>::apply(c.x, d1.x, u1.x);
+    s1 += StencilZ<S_LAP5>::apply(c.y, d1.y, u1.y);
+  }
+}
+// ... of one cell with the boundary rule along z; oc = offset of the cell inside its plane
+template <int STENCIL>
+CARDIAC_D double zarm_edge(const double* __restrict__ U, int oc, int kz, int nz, int zs, int bc, double c) {
+  const double d1 = U[(long long)bidx(kz - 1, nz, bc) * zs + oc], u1 = U[(long long)bidx(kz + 1, nz, bc) * zs + oc];
+  if (STENCIL == S_LAP9X4) {
+    const double d2 = U[(long long)bidx(kz - 2, nz, bc) * zs + oc], u2 = U[(long long)bidx(kz + 2, nz, bc) * zs + oc];
+    return StencilZ<S_LAP9X4>::apply(c, d1, u1, d2, u2);
+  } else if (STENCIL == S_LAP5) {
+    return StencilZ<S_LAP5>::apply(c, d1, u1);
+  }
+  return 0.0;
+}
+
 // the update of one cell once f = D lap + N is known; o = offset of the cell inside its field
 template <class MD, int KIND>
 CARDIAC_D void finish_cell(const StageArgs<MD>& a, const double* __restrict__ yb,
                            const double* __restrict__ Ab, const double* __restrict__ Bb,
-                           double* __restrict__ ob, int o, const double (&z)[MD::NV],
+                           double* __restrict__ ob, long long o, const double (&z)[MD::NV],
                            const double (&f)[MD::NV]) {
   constexpr int NV = MD::NV;
   if (KIND == K_RL || KIND == K_IE) {
@@ -79,7 +109,7 @@ CARDIAC_D void finish_cell(const StageArgs<MD>& a, const double* __restrict__ yb
   }
 }
 
-template <class MD, int STENCIL, int KIND>
+template <class MD, int STENCIL, int KIND, bool D3>
 __global__ void __launch_bounds__(TX* TY, 4)
     stage_kernel(const __grid_constant__ StageArgs<MD> a) {
   constexpr int NV = MD::NV, ND = MD::ND;
@@ -87,7 +117,11 @@ __global__ void __launch_bounds__(TX* TY, 4)
   const int nx = a.g.nx, ny = a.g.ny, pitch = a.g.pitch;
   const int x0 = blockIdx.x * (2 * TX), j0 = blockIdx.y * TY;
   const int x = x0 + 2 * threadIdx.x, j = j0 + threadIdx.y;
-  const long long base = (long long)blockIdx.z * a.g.bstride;
+  // 2-D: blockIdx.z = batch member.  3-D: blockIdx.z = member * nz + plane
+  const int kz = D3 ? (int)(blockIdx.z % a.g.nz) : 0;
+  typedef typename Off<D3>::type off_t;
+  const off_t pz = D3 ? (off_t)kz * a.g.zstride : 0;            // offset of the plane inside a field
+  const long long base = (long long)(D3 ? blockIdx.z / a.g.nz : blockIdx.z) * a.g.bstride;
   const double* __restrict__ in = a.in + base;
   const double* __restrict__ yb = a.y + base;
   const double* __restrict__ Ab = a.A + base;
@@ -95,9 +129,11 @@ __global__ void __launch_bounds__(TX* TY, 4)
   double* __restrict__ ob = a.out + base;
 
   // block-uniform: tile and halo inside the grid -> no boundary logic, 128-bit accesses
-  const bool interior = x0 >= 2 && x0 + 2 * TX + 2 <= nx && j0 >= R && j0 + TY + R <= ny;
+  const bool interior = x0 >= 2 && x0 + 2 * TX + 2 <= nx && j0 >= R && j0 + TY + R <= ny &&
+                        (!D3 || (kz >= R && kz + R < a.g.nz));
   if (interior && KIND != K_RL && KIND != K_IE) {
-    const int row = j * pitch, o = row + x;
+    const int row = j * pitch;
+    const off_t o = pz + row + x;
     // The gating fields are first used ~400 instructions into the reaction and y at its very end;
     // under the 64-register cap ptxas sinks those loads next to their use (a second and third exposed
     // latency per warp).  Asking L1 for the lines now costs no register; the late loads then hit.
@@ -122,7 +158,10 @@ __global__ void __launch_bounds__(TX* TY, 4)
     // than keeping 12 more 128-bit loads in flight per thread (or prefetching them to L1).
     double s0[ND], s1[ND];
 #pragma unroll
-    for (int q = 0; q < ND; ++q) stencil_pair<STENCIL>(in + q * a.g.fstride, row, x, pitch, zz[q], s0[q], s1[q]);
+    for (int q = 0; q < ND; ++q) {
+      stencil_pair<STENCIL>(in + q * a.g.fstride + pz, row, x, pitch, zz[q], s0[q], s1[q]);
+      if (D3) zarm_pair<STENCIL>(in + q * a.g.fstride, o, a.g.zstride, zz[q], s0[q], s1[q]);
+    }
     double z0[NV], z1[NV], f0[NV], f1[NV];
 #pragma unroll
     for (int q = 0; q < NV; ++q) { z0[q] = zz[q].x; z1[q] = zz[q].y; }
@@ -152,14 +191,16 @@ __global__ void __launch_bounds__(TX* TY, 4)
   for (int h = 0; h < 2; ++h) {
     const int i = x + h;
     if (i >= nx) break;
-    const int o = j * pitch + i;
+    const int oc = j * pitch + i;        // inside the plane
+    const off_t o = pz + oc;             // inside the field
     double z[NV], f[NV];
 #pragma unroll
     for (int q = 0; q < NV; ++q) z[q] = in[o + q * a.g.fstride];
     MD::reaction(a.p, z, f);
 #pragma unroll
     for (int q = 0; q < ND; ++q) {
-      double s = stencil_edge<STENCIL>(in + q * a.g.fstride, i, j, nx, ny, pitch, bc, z[q]);
+      double s = stencil_edge<STENCIL>(in + q * a.g.fstride + pz, i, j, nx, ny, pitch, bc, z[q]);
+      if (D3) s += zarm_edge<STENCIL>(in + q * a.g.fstride, oc, kz, a.g.nz, a.g.zstride, bc, z[q]);
       f[q] = fma(a.lapw[q], s, f[q]);
     }
     finish_cell<MD, KIND>(a, yb, Ab, Bb, ob, o, z, f);
@@ -173,13 +214,19 @@ cudaError_t run(const Problem& pb, const StageLaunch& st, cudaStream_t stream) {
   a.in = st.in; a.y = st.y ? st.y : st.in; a.A = st.A ? st.A : st.in; a.B = st.B ? st.B : st.in;
   a.out = st.out;
   a.g.nx = pb.nx; a.g.ny = pb.ny; a.g.pitch = pb.pitch; a.g.boundary = pb.boundary;
+  a.g.nz = pb.nz; a.g.zstride = pb.zstride;
   a.g.fstride = pb.fstride; a.g.bstride = pb.bstride;
   a.w_y = st.w_y; a.w_in = st.w_in; a.w_A = st.w_A; a.w_B = st.w_B; a.w_f = st.w_f;
   a.dt = pb.dt;
   MD::derive(pb.params, a.p);
   for (int q = 0; q < MD::ND; ++q) a.lapw[q] = a.p.D[q] * stencil_norm(STENCIL) / (pb.dx * pb.dx);
-  dim3 grid((pb.nx + 2 * TX - 1) / (2 * TX), (pb.ny + TY - 1) / TY, pb.batch), block(TX, TY);
-  stage_kernel<MD, STENCIL, KIND><<<grid, block, 0, stream>>>(a);
+  dim3 grid((pb.nx + 2 * TX - 1) / (2 * TX), (pb.ny + TY - 1) / TY, pb.batch * pb.nz), block(TX, TY);
+  if (pb.nz > 1) {
+    if constexpr (STENCIL == S_BOX9) return cudaErrorInvalidValue;   // no 3-D counterpart (rejected at create)
+    else stage_kernel<MD, STENCIL, KIND, true><<<grid, block, 0, stream>>>(a);
+  } else {
+    stage_kernel<MD, STENCIL, KIND, false><<<grid, block, 0, stream>>>(a);
+  }
   return cudaGetLastError();
 }
 
@@ -246,9 +293,9 @@ cudaError_t launch_stage(const Problem& pb, const StageLaunch& st, cudaStream_t 
 
 cudaError_t launch_jvp(const Problem& pb, const double* state, double eps, double* dst,
                        cudaStream_t stream) {
-  const long long n = (long long)pb.nx * pb.ny * pb.nv;
+  const long long n = (long long)pb.nx * pb.ny * pb.nz * pb.nv;
   dim3 grid((unsigned)((n + 255) / 256), pb.batch - 1);
-  jvp_kernel<<<grid, 256, 0, stream>>>(state, dst, pb.nx, pb.ny, pb.nv, pb.pitch, pb.bstride, eps);
+  jvp_kernel<<<grid, 256, 0, stream>>>(state, dst, pb.nx, pb.ny * pb.nz, pb.nv, pb.pitch, pb.bstride, eps);
   return cudaGetLastError();
 }
 

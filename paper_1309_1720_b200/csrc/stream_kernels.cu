@@ -353,6 +353,7 @@ cudaError_t run_ring(const Problem& pb, const StageLaunch& st, cudaStream_t stre
   a.in = st.in; a.y = st.y ? st.y : st.in; a.A = st.A ? st.A : st.in; a.B = st.B ? st.B : st.in;
   a.out = st.out;
   a.g.nx = pb.nx; a.g.ny = pb.ny; a.g.pitch = pb.pitch; a.g.boundary = pb.boundary;
+  a.g.nz = 1; a.g.zstride = pb.zstride;
   a.g.fstride = pb.fstride; a.g.bstride = pb.bstride;
   a.w_y = st.w_y; a.w_in = st.w_in; a.w_A = st.w_A; a.w_B = st.w_B; a.w_f = st.w_f;
   a.dt = pb.dt;
@@ -409,6 +410,7 @@ cudaError_t ring_by_stencil(const Problem& pb, const StageLaunch& st, cudaStream
 
 bool stage_ring_supported(const Problem& pb, int kind) {
   if (kind != K_SELF && kind != K_BASE && kind != K_RK4F) return false;
+  if (pb.nz > 1) return false;   // the ring tiles are 2-D
   // tensor-map limits: strides are multiples of 16 bytes by construction (pitch % 16 == 0)
   const long long ntiles = (long long)((pb.nx + TW - 1) / TW) * ((pb.ny + TH - 1) / TH) * pb.batch;
   return ntiles < (1LL << 31) && encoder() != nullptr;

@@ -41,6 +41,7 @@ __global__ void __launch_bounds__(TG::NT, TG::MINB)
 template <class MD>
 void fill_tile_args(const Problem& pb, int stencil, TileArgs<MD>& a) {
   a.g.nx = pb.nx; a.g.ny = pb.ny; a.g.pitch = pb.pitch; a.g.boundary = pb.boundary;
+  a.g.nz = 1; a.g.zstride = pb.zstride;
   a.g.fstride = pb.fstride; a.g.bstride = pb.bstride;
   const double dt = pb.dt;
   for (int s = 0; s < 4; ++s) a.a_dt[s] = a.b_dt[s] = 0.0;

@@ -106,6 +106,7 @@ class Config:
     dt: float = 0.0
     boundary: int = 0   # 0 no-flux, 1 periodic
     variant: int = 0    # 0 as printed, 1 tanh-free
+    nz: int = 1         # > 1: 3-D grid [nz][ny][nx] (DESIGN.md f4)
 
     @property
     def n_v(self) -> int:
@@ -117,7 +118,7 @@ class Config:
 
     @property
     def cells(self) -> int:
-        return self.nx * self.ny * self.batch
+        return self.nx * self.ny * self.nz * self.batch
 
     def describe(self) -> str:
         return (f"{self.name}: {MODEL_NAMES[self.model]} {self.batch}x{self.ny}x{self.nx} "
@@ -280,8 +281,29 @@ def sweep_state(cfg: Config, base: int = 256) -> np.ndarray:
     return np.ascontiguousarray(z)
 
 
+def state_3d(cfg: Config) -> np.ndarray:
+    """3-D input: the block-noise recipe of config 3 per plane (a different seed per plane), then five
+    averaging sweeps along z with mirrored ends, dense [batch][n_v][nz][ny][nx]."""
+    planes = [state_blocks(replace(cfg, nz=1, batch=1), seed=cfg.seed + 31 * k)[0] for k in range(cfg.nz)]
+    z = np.stack(planes, axis=1)                     # [n_v][nz][ny][nx]
+    for _ in range(5):
+        p = np.pad(z, ((0, 0), (1, 1), (0, 0), (0, 0)), mode="reflect")
+        z = 0.5 * z + 0.25 * (p[:, :-2] + p[:, 2:])
+    out = np.repeat(z[None], cfg.batch, axis=0)
+    if cfg.batch > 1:
+        out[1:] += 1e-3 * gaussian(cfg.seed + 77, out[1:].size).reshape(out[1:].shape)
+    return np.ascontiguousarray(out)
+
+
+def default_dt_3d(model: int) -> float:
+    """Half the explicit limit of the 7-point stencil, dx^2 / (6 D_max)."""
+    return 0.5 * DX[model] ** 2 / (6.0 * D_MAX[model])
+
+
 def initial_state(cfg: Config) -> np.ndarray:
     """Initial state of a (possibly scaled) baseline config, dense [batch][n_v][ny][nx]."""
+    if cfg.nz > 1:
+        return state_3d(cfg)
     base = cfg.name.split("@")[0]
     if base == "cfg1":
         return state_cfg1(cfg)

@@ -66,3 +66,22 @@ def test_initial_states():
     d = (z[1:] - z[0]) / 1e-7
     assert np.allclose(np.sqrt(np.sum(d ** 2, axis=(1, 2, 3))), 1.0, atol=1e-6)
     assert abs(np.sum(d[0] * d[1])) < 0.2                 # different directions
+
+
+def test_sweep_and_3d_inputs():
+    """Size sweep S and the 3-D inputs: shapes, determinism, value ranges."""
+    assert W.sweep_sizes()[0] == 64 and 362 in W.sweep_sizes() and W.sweep_sizes()[-1] == 8192
+    c = W.sweep_config(W.KARMA, 362)
+    assert (c.stencil, c.integrator, c.nsteps) == (W.LAP5, W.RK4, 200) and W.sweep_config(W.BOCF, 8192).nsteps == 32
+    z = W.sweep_state(c)
+    assert z.shape == (1, 2, 362, 362) and np.array_equal(z, W.sweep_state(c))
+    assert np.array_equal(z[0, :, :106, :106], z[0, :, 256:362, 256:362])     # the 256^2 base, repeated
+    lo, hi = W.U_RANGE[W.KARMA]
+    assert lo <= z[0, 0].min() and z[0, 0].max() <= hi
+    c3 = W.make_config("v", W.BOCF, 20, W.LAP9X4, W.RK4, 0, batch=2, seed=4, ny=12, nz=7)
+    assert c3.cells == 2 * 20 * 12 * 7
+    z3 = W.initial_state(c3)
+    assert z3.shape == (2, 4, 7, 12, 20) and np.array_equal(z3, W.initial_state(c3))
+    assert not np.array_equal(z3[0, 0, 0], z3[0, 0, 3])                        # planes differ
+    assert 0 < np.max(np.abs(z3[1] - z3[0])) < 1e-2                             # perturbed batch member
+    assert W.default_dt_3d(W.FHN) == pytest.approx(0.5 * 0.04 ** 2 / (6 * 1.5), rel=1e-15)

@@ -106,24 +106,36 @@ struct TileEngine {
     const int gx = bx * TW - H + 2 * tx;
     const int gy0 = by * TH - H + PR * ty;
     const bool vec = VEC && gx >= 0 && gx + 1 < nx;
-    const int fx0 = fold(gx, nx, bc), fx1 = fold(gx + 1, nx, bc);
+    // A window reaches at most H cells (plus the ragged part of the last tile) outside the grid: when
+    // the grid is larger than that, ONE reflection / wrap maps every index (no integer division —
+    // the general fold() was a quarter of all instructions of the kernel, ncu r1 v5).
+    const bool once_x = nx > H + TW, once_y = ny > H + TH;
+    const int fx0 = once_x ? bidx(gx, nx, bc) : fold(gx, nx, bc);
+    const int fx1 = once_x ? bidx(gx + 1, nx, bc) : fold(gx + 1, nx, bc);
     double* s0 = sm + (R + PR * ty) * SP + PADX + 2 * tx;
+    // all loads first, then the stores: one exposed memory latency per thread instead of one per row
+    double2 v[PR][NV];
 #pragma unroll
     for (int k = 0; k < PR; ++k) {
-      const int row = fold(gy0 + k, ny, bc) * pitch;
+      const int row = (once_y ? bidx(gy0 + k, ny, bc) : fold(gy0 + k, ny, bc)) * pitch;
 #pragma unroll
       for (int q = 0; q < NV; ++q) {
         const double* f = in + q * a.g.fstride + row;
-        double2 v;
         if (vec) {
-          v = *reinterpret_cast<const double2*>(f + gx);
+          v[k][q] = *reinterpret_cast<const double2*>(f + gx);
         } else {
-          v.x = f[fx0];
-          v.y = f[fx1];
+          v[k][q].x = f[fx0];
+          v[k][q].y = f[fx1];
         }
-        if (q < ND) *reinterpret_cast<double2*>(s0 + q * FSZ + k * SP) = v;
-        else { st.g[k][0][q - ND] = v.x; st.g[k][1][q - ND] = v.y; }
-        if (RK) { st.y[k][0][q] = v.x; st.y[k][1][q] = v.y; }
+      }
+    }
+#pragma unroll
+    for (int k = 0; k < PR; ++k) {
+#pragma unroll
+      for (int q = 0; q < NV; ++q) {
+        if (q < ND) *reinterpret_cast<double2*>(s0 + q * FSZ + k * SP) = v[k][q];
+        else { st.g[k][0][q - ND] = v[k][q].x; st.g[k][1][q - ND] = v[k][q].y; }
+        if (RK) { st.y[k][0][q] = v[k][q].x; st.y[k][1][q] = v[k][q].y; }
       }
     }
   }

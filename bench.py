@@ -199,7 +199,7 @@ def run_reference(args, cfg, rank):
     }))
 
 
-PLAN_NAMES = {1: "stage", 2: "fused", 3: "persistent"}
+PLAN_NAMES = {1: "stage", 2: "fused", 3: "persistent", 4: "pair"}
 
 
 def time_config(C, torch, cfg, Z0, steps, warmup, flush, plan=0, plan_param=0):

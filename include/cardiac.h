@@ -68,10 +68,14 @@ enum {
   CARDIAC_PLAN_STAGE      = 1, /* one fused stencil+reaction+RK-stage launch per substep        */
   CARDIAC_PLAN_FUSED      = 2, /* all substeps of one time step (or several Euler steps) on chip,
                                   overlapped tiles, one launch                                  */
-  CARDIAC_PLAN_PERSISTENT = 3  /* ONE launch for all nsteps: each batch member resident in the shared
+  CARDIAC_PLAN_PERSISTENT = 3, /* ONE launch for all nsteps: each batch member resident in the shared
                                   memory of a thread-block cluster (<= 8 CTAs), ghost rows exchanged
                                   through distributed shared memory; grids up to 8 x 4096 cells
                                   (4-field model: 8 x 2048); Euler, Heun, RK4                   */
+  CARDIAC_PLAN_PAIR       = 4  /* two consecutive substeps per launch: the first on tile + ring into
+                                  shared memory, the second from there (RK4: two launches, the fourth
+                                  stage value never reaches memory; Heun: one launch; Euler: two time
+                                  steps per launch); 2-D; Euler, Heun, RK4                      */
 };
 
 /* error codes */
@@ -129,7 +133,8 @@ int cardiac_set_stream(cardiac_ctx*, void* cuda_stream);
  * launch (0 = default); FUSED + Heun/RK4 = window (0 = by size, 1 = 80x48 cells, one CTA per SM,
  * 2 = 48x40 cells, two CTAs per SM, two-field models only); STAGE = kernel implementation (0 = by size, 1 = DIRECT: every thread loads
  * its own operands, 2 = RING: persistent CTAs fed by a TMA shared-memory ring; same results
- * bitwise); otherwise 0. */
+ * bitwise); PAIR, PERSISTENT: 0.  AUTO: PERSISTENT below ~100x100 cells per member, FUSED for the
+ * two-field models, PAIR for the four-field model with Heun / RK4 from 12 Mi cells, else STAGE. */
 int cardiac_set_plan(cardiac_ctx*, int plan, int param);
 
 /* The plan that cardiac_step will use (resolved from AUTO). */

@@ -25,7 +25,7 @@ CARDIAC_EULER, CARDIAC_HEUN, CARDIAC_RK4 = 0 << 8, 1 << 8, 2 << 8
 CARDIAC_RUSH_LARSEN, CARDIAC_IMPLICIT_EULER = 3 << 8, 4 << 8
 CARDIAC_NOFLUX, CARDIAC_PERIODIC = 0 << 16, 1 << 16
 CARDIAC_VARIANT_PAPER, CARDIAC_VARIANT_TANHFREE = 0 << 24, 1 << 24
-CARDIAC_PLAN_AUTO, CARDIAC_PLAN_STAGE, CARDIAC_PLAN_FUSED, CARDIAC_PLAN_PERSISTENT = 0, 1, 2, 3
+CARDIAC_PLAN_AUTO, CARDIAC_PLAN_STAGE, CARDIAC_PLAN_FUSED, CARDIAC_PLAN_PERSISTENT, CARDIAC_PLAN_PAIR = 0, 1, 2, 3, 4
 CARDIAC_PROBE_EXP, CARDIAC_PROBE_RCP, CARDIAC_PROBE_HK, CARDIAC_PROBE_REACTION = 0, 1, 2, 3
 CARDIAC_OK, CARDIAC_ERR_INVALID, CARDIAC_ERR_CUDA, CARDIAC_ERR_NOSTATE, CARDIAC_ERR_WORKSPACE = 0, -1, -2, -3, -4
 

@@ -37,7 +37,7 @@ struct cardiac_ctx {
   double* buf[kMaxBuf] = {nullptr, nullptr, nullptr, nullptr};
   int cur = 0;  // buffer holding the state
   bool has_state = false;
-  cudaGraphExec_t graph[2] = {nullptr, nullptr};  // keyed by `cur` parity at graph start
+  cudaGraphExec_t graph[kMaxBuf] = {nullptr, nullptr, nullptr, nullptr};  // keyed by `cur` at graph start
   int graph_steps = 0;
   long long launches = 0;
   std::string err;
@@ -98,6 +98,12 @@ int auto_plan(const Problem& pb) {
   if (pb.nz > 1) return CARDIAC_PLAN_STAGE;   // 3-D: the stage-synchronous plan only
   if (resident_preferred(pb)) return CARDIAC_PLAN_PERSISTENT;
   if (rk_like && pb.model != CARDIAC_BOCF) return CARDIAC_PLAN_FUSED;
+  // 4-field model, Heun / RK4: two substeps per launch once the grid gives every SM >= ~20 waves of
+  // tiles (measured on B200: 4096^2 +5 %, 8192^2 +11 % over STAGE; at 2048^2 the
+  // 6.2 waves of 64 x 24 tiles lose 5 % to the last partial wave)
+  if (pb.model == CARDIAC_BOCF && (pb.integrator == I_HEUN || pb.integrator == I_RK4) &&
+      (long long)pb.nx * pb.ny * pb.batch >= kPairMinCells)
+    return CARDIAC_PLAN_PAIR;
   return CARDIAC_PLAN_STAGE;
 }
 
@@ -108,22 +114,83 @@ bool fused_small(const cardiac_ctx* c) {
 
 // Plan FUSED: one launch advances `ksteps` time steps (1, or kEulerBlock Euler steps), ping-pong.
 int enqueue_fused(cardiac_ctx* c, cudaStream_t s, int ksteps) {
-  TileLaunch tl{c->buf[c->cur], c->buf[1 - c->cur], ksteps, fused_small(c)};
+  const int other = c->cur == 0 ? 1 : 0;   // (plan PAIR may have left the state in buffer 2)
+  TileLaunch tl{c->buf[c->cur], c->buf[other], ksteps, fused_small(c)};
   cudaError_t e = launch_fused(c->pb, tl, s);
   if (e != cudaSuccess) return fail_cuda(c, e, "fused launch");
   c->launches++;
-  c->cur ^= 1;
+  c->cur = other;
+  return CARDIAC_OK;
+}
+
+// Plan PAIR: buffers the state rotates through (RK4: y, Y2, Y3 — Y4 never leaves the SM)
+int pair_ring(const cardiac_ctx* c) { return c->pb.integrator == I_RK4 ? 3 : 2; }
+
+// Plan PAIR: one time step (Heun, RK4) or two (Euler) in one or two launches of two substeps each.
+int enqueue_pair(cardiac_ctx* c, cudaStream_t s) {
+  const Problem& pb = c->pb;
+  const double dt = pb.dt;
+  const int ring = pair_ring(c);
+  const int n1 = c->cur < ring ? (c->cur + 1) % ring : 0, n2 = (n1 + 1) % ring;
+  double* b0 = c->buf[c->cur];
+  double* b1 = c->buf[n1];
+  auto go = [&](const PairLaunch& pl) -> int {
+    cudaError_t e = launch_pair(pb, pl, s);
+    if (e != cudaSuccess) return fail_cuda(c, e, "pair launch");
+    c->launches++;
+    return CARDIAC_OK;
+  };
+  int rc = CARDIAC_OK;
+  PairLaunch pl{};
+  pl.in = b0; pl.y = b0;
+  switch (pb.integrator) {
+    case I_EULER:   // y1 = y + dt f(y) [on chip]; y2 = y1 + dt f(y1)
+      pl.ka = K_SELF; pl.kb = K_SELF; pl.out = b1; pl.a_wf = dt; pl.w_f = dt;
+      rc = go(pl);
+      break;
+    case I_HEUN:    // Y2 = y + dt f(y) [on chip]; y+ = (y + Y2)/2 + dt/2 f(Y2)
+      pl.ka = K_SELF; pl.kb = K_BASE; pl.out = b1; pl.a_wf = dt;
+      pl.w_y = 0.5; pl.w_in = 0.5; pl.w_f = 0.5 * dt;
+      rc = go(pl);
+      break;
+    case I_RK4: {   // same combinations and weights as plan STAGE (enqueue_step)
+      double* b2 = c->buf[n2];
+      pl.ka = K_SELF; pl.kb = K_BASE; pl.mid = b1; pl.out = b2; pl.a_wf = 0.5 * dt;
+      pl.w_y = 1.0; pl.w_in = 0.0; pl.w_f = 0.5 * dt;
+      if ((rc = go(pl))) break;
+      pl = PairLaunch{};
+      pl.ka = K_BASE; pl.kb = K_RK4F; pl.in = b2; pl.y = b0; pl.A = b1; pl.B = b2; pl.out = b1;
+      pl.a_wy = 1.0; pl.a_win = 0.0; pl.a_wf = dt;
+      pl.w_y = -1.0 / 3.0; pl.w_in = 1.0 / 3.0; pl.w_A = 1.0 / 3.0; pl.w_B = 2.0 / 3.0; pl.w_f = dt / 6.0;
+      rc = go(pl);
+      break;
+    }
+    default:
+      return fail(c, CARDIAC_ERR_INVALID, "PAIR supports Euler, Heun and RK4 only");
+  }
+  if (rc) return rc;
+  c->cur = n1;
   return CARDIAC_OK;
 }
 
 // time steps advanced by one repetition unit of the plan
 int unit_steps(const cardiac_ctx* c) {
+  if (c->plan == CARDIAC_PLAN_PAIR) return c->pb.integrator == I_EULER ? 2 : 1;
   return (c->plan == CARDIAC_PLAN_FUSED && c->pb.integrator == I_EULER) ? c->plan_param : 1;
+}
+
+// one repetition unit of the plan (unit_steps time steps)
+int enqueue_step(cardiac_ctx* c, cudaStream_t s);
+int enqueue_unit(cardiac_ctx* c, cudaStream_t s) {
+  if (c->plan == CARDIAC_PLAN_PAIR) return enqueue_pair(c, s);
+  const int us = unit_steps(c);
+  return us == 1 ? enqueue_step(c, s) : enqueue_fused(c, s, us);
 }
 
 // Enqueue the kernels of ONE time step on `s`; advances c->cur as the real execution would.
 int enqueue_step(cardiac_ctx* c, cudaStream_t s) {
   if (c->plan == CARDIAC_PLAN_FUSED) return enqueue_fused(c, s, 1);
+  if (c->plan == CARDIAC_PLAN_PAIR && c->pb.integrator != I_EULER) return enqueue_pair(c, s);
   const Problem& pb = c->pb;
   const double dt = pb.dt;
   StageLaunch st{};
@@ -149,7 +216,8 @@ int enqueue_step(cardiac_ctx* c, cudaStream_t s) {
     case I_IMPLICIT_EULER: {
       int kind = pb.integrator == I_EULER ? K_SELF : (pb.integrator == I_RUSH_LARSEN ? K_RL : K_IE);
       rc = go(kind, b[0], nullptr, nullptr, nullptr, b[1], 0, 0, 0, 0, dt);
-      c->cur ^= 1;
+      for (int i = 0; i < c->nbuf; ++i)
+        if (c->buf[i] == b[1]) c->cur = i;
       break;
     }
     case I_HEUN:
@@ -178,15 +246,18 @@ int build_graph(cardiac_ctx* c, int units) {
   long long launches_before = c->launches;
   CK(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
   int rc = CARDIAC_OK;
-  const int us = unit_steps(c);
-  for (int s = 0; s < units && rc == CARDIAC_OK; ++s)
-    rc = us == 1 ? enqueue_step(c, c->cap_stream) : enqueue_fused(c, c->cap_stream, us);
+  for (int s = 0; s < units && rc == CARDIAC_OK; ++s) rc = enqueue_unit(c, c->cap_stream);
+  const int end_cur = c->cur;
   cudaGraph_t g = nullptr;
   cudaError_t e = cudaStreamEndCapture(c->cap_stream, &g);
   c->cur = parity;  // capture executed nothing
   c->launches = launches_before;
   if (rc != CARDIAC_OK) { if (g) cudaGraphDestroy(g); return rc; }
   if (e != cudaSuccess) return fail_cuda(c, e, "cudaStreamEndCapture");
+  if (end_cur != parity) {   // a graph is replayed back to back: it must end in the buffer it started from
+    cudaGraphDestroy(g);
+    return fail(c, CARDIAC_ERR_INVALID, "internal: graph does not return to its start buffer");
+  }
   e = cudaGraphInstantiate(&c->graph[parity], g, 0);
   cudaGraphDestroy(g);
   if (e != cudaSuccess) return fail_cuda(c, e, "cudaGraphInstantiate");
@@ -370,6 +441,9 @@ int cardiac_set_plan(cardiac_ctx* c, int plan, int param) {
                     "FUSED + Heun/RK4: parameter 0 (auto), 1 (80x48 window) or 2 (48x40 window, 2-field models)");
       rparam = param == 0 ? fused_window_auto(c->pb) : param;
     }
+  } else if (resolved == CARDIAC_PLAN_PAIR) {
+    if (!rk_like) return fail(c, CARDIAC_ERR_INVALID, "PAIR supports Euler, Heun and RK4 only");
+    if (param != 0) return fail(c, CARDIAC_ERR_INVALID, "plan parameter must be 0");
   } else if (resolved == CARDIAC_PLAN_PERSISTENT) {
     if (!resident_supported(c->pb))
       return fail(c, CARDIAC_ERR_INVALID,
@@ -451,9 +525,11 @@ int cardiac_step(cardiac_ctx* c, long long nsteps) {
     return CARDIAC_OK;
   }
   const int us = unit_steps(c);                                        // time steps per unit
-  const int ul = c->plan == CARDIAC_PLAN_FUSED ? 1 : stages_of(c->pb.integrator);  // launches per unit
+  const int ul = c->plan == CARDIAC_PLAN_FUSED ? 1   // launches per unit
+                 : (c->plan == CARDIAC_PLAN_PAIR ? (c->pb.integrator == I_RK4 ? 2 : 1) : stages_of(c->pb.integrator));
   int gunits = kGraphNodes / ul;
   if (gunits & 1) gunits++;  // even: ping-pong plans end on the parity they started on
+  if (c->plan == CARDIAC_PLAN_PAIR) gunits = gunits / 6 * 6;   // ... and the rotation through 2 or 3 buffers
   const long long gsteps = (long long)gunits * us;
   long long left = nsteps;
   if (left >= gsteps) {
@@ -469,7 +545,7 @@ int cardiac_step(cardiac_ctx* c, long long nsteps) {
     }
   }
   for (; left >= us; left -= us) {
-    int rc = us == 1 ? enqueue_step(c, c->stream) : enqueue_fused(c, c->stream, us);
+    int rc = enqueue_unit(c, c->stream);
     if (rc) return rc;
   }
   for (; left > 0; --left) {  // fewer Euler steps than one temporal block

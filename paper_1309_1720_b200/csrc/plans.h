@@ -58,6 +58,30 @@ inline cudaError_t launch_fused(const Problem& pb, const TileLaunch& tl, cudaStr
                                         : launch_fused_bocf(pb, tl, stream));
 }
 
+// pair_kernels_*.cu: plan PAIR — two consecutive substeps per launch (pair.cuh): substep A (ka =
+// K_SELF or K_BASE) on tile + ring into shared memory (and into `mid` when not null), substep B (kb)
+// on the tile from shared memory into `out`.  out != in, out != y; out == A allowed.
+struct PairLaunch {
+  int ka, kb;
+  const double* in;
+  const double* y;
+  const double* A;
+  const double* B;
+  double* mid;
+  double* out;
+  double a_wy, a_win, a_wf;
+  double w_y, w_in, w_A, w_B, w_f;
+};
+constexpr long long kPairMinCells = 12LL << 20;  // AUTO: 4-field model, Heun / RK4
+cudaError_t launch_pair_fhn(const Problem& pb, const PairLaunch& pl, cudaStream_t stream);
+cudaError_t launch_pair_karma(const Problem& pb, const PairLaunch& pl, cudaStream_t stream);
+cudaError_t launch_pair_bocf(const Problem& pb, const PairLaunch& pl, cudaStream_t stream);
+inline cudaError_t launch_pair(const Problem& pb, const PairLaunch& pl, cudaStream_t stream) {
+  return pb.model == 0 ? launch_pair_fhn(pb, pl, stream)
+                       : (pb.model == 1 ? launch_pair_karma(pb, pl, stream)
+                                        : launch_pair_bocf(pb, pl, stream));
+}
+
 // resident_kernels_*.cu: plan PERSISTENT — one thread-block cluster of C <= 8 CTAs per batch member
 // keeps the whole grid in (distributed) shared memory and advances all nsteps in ONE launch, in place
 // (resident.cuh).  C CTAs of 512 threads x KP pairs: at most C x 4096 cells (2-field models) or

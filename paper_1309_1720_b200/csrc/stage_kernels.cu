@@ -25,26 +25,6 @@ constexpr int TX = 32, TY = 8;   // threads; the tile is 2*TX x TY cells
 template <bool D3> struct Off { typedef int type; };
 template <> struct Off<true> { typedef long long type; };
 
-// one cell with the boundary rule applied per axis (Q3)
-template <int STENCIL>
-CARDIAC_D double stencil_edge(const double* __restrict__ U, int i, int j, int nx, int ny, int pitch,
-                              int bc, double c) {
-  const int rw1 = bidx(i - 1, nx, bc), re1 = bidx(i + 1, nx, bc);
-  const int row = j * pitch;
-  const int rs1 = bidx(j - 1, ny, bc) * pitch, rn1 = bidx(j + 1, ny, bc) * pitch;
-  if (STENCIL == S_LAP5) {
-    return Stencil<S_LAP5>::apply(c, U[row + rw1], U[row + re1], U[rs1 + i], U[rn1 + i]);
-  } else if (STENCIL == S_LAP9X4) {
-    const int rw2 = bidx(i - 2, nx, bc), re2 = bidx(i + 2, nx, bc);
-    const int rs2 = bidx(j - 2, ny, bc) * pitch, rn2 = bidx(j + 2, ny, bc) * pitch;
-    return Stencil<S_LAP9X4>::apply(c, U[row + rw1], U[row + re1], U[rs1 + i], U[rn1 + i],
-                                    U[row + rw2], U[row + re2], U[rs2 + i], U[rn2 + i]);
-  } else {
-    return Stencil<S_BOX9>::apply(c, U[row + rw1], U[row + re1], U[rs1 + i], U[rn1 + i],
-                                  U[rs1 + rw1], U[rs1 + re1], U[rn1 + rw1], U[rn1 + re1]);
-  }
-}
-
 // 3-D: the z arm of the pair (x, x+1) at offset o of a field, planes kz +- m inside the grid
 template <int STENCIL>
 CARDIAC_D void zarm_pair(const double* __restrict__ U, long long o, int zs, double2 c, double& s0, double& s1) {

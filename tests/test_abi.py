@@ -49,7 +49,7 @@ def test_enums_match_header(C):
     src = open(os.path.join(ROOT, "include", "cardiac.h")).read()
     for name in ("CARDIAC_FHN", "CARDIAC_KARMA", "CARDIAC_BOCF", "CARDIAC_LAP5", "CARDIAC_LAP9X4",
                  "CARDIAC_BOX9", "CARDIAC_PLAN_AUTO", "CARDIAC_PLAN_STAGE", "CARDIAC_PLAN_FUSED",
-                 "CARDIAC_PLAN_PERSISTENT", "CARDIAC_OK", "CARDIAC_ERR_INVALID", "CARDIAC_ERR_CUDA",
+                 "CARDIAC_PLAN_PERSISTENT", "CARDIAC_PLAN_PAIR", "CARDIAC_OK", "CARDIAC_ERR_INVALID", "CARDIAC_ERR_CUDA",
                  "CARDIAC_ERR_NOSTATE", "CARDIAC_ERR_WORKSPACE"):
         m = re.search(rf"\b{name}\s*=\s*(-?\d+)", src)
         assert m and int(m.group(1)) == getattr(C, name), name

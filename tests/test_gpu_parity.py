@@ -56,9 +56,10 @@ CASES += [(BOCF, s, i) for s in (LAP5, LAP9X4, BOX9) for i in (RL, IE)]
 
 # CARDIAC_PLAN_* (+ parameter): STAGE with its DIRECT kernels, STAGE with the TMA-ring kernels
 # (forced: AUTO would pick DIRECT at these oracle-sized grids), FUSED
-STAGE, RING, FUSED, PERSISTENT = (1, 1), (1, 2), 2, 3
+# PAIR (two substeps per launch)
+STAGE, RING, FUSED, PERSISTENT, PAIR = (1, 1), (1, 2), 2, 3, 4
 PLAN_CASES = [(m, s, i, STAGE) for (m, s, i) in CASES]
-PLAN_CASES += [(m, s, i, p) for (m, s, i) in CASES if i in (EULER, HEUN, RK4) for p in (RING, FUSED)]
+PLAN_CASES += [(m, s, i, p) for (m, s, i) in CASES if i in (EULER, HEUN, RK4) for p in (RING, FUSED, PAIR)]
 
 
 @pytest.mark.parametrize("model,stencil,integ,plan", PLAN_CASES)
@@ -149,7 +150,7 @@ def test_persistent_plan_limits_and_auto(C):
 
 @pytest.mark.parametrize("model,stencil,integ", [(FHN, LAP9X4, RK4), (KARMA, LAP5, RK4), (BOCF, LAP9X4, RK4),
                                                  (FHN, LAP5, EULER), (BOCF, BOX9, HEUN)])
-@pytest.mark.parametrize("plan", [STAGE, RING, FUSED])
+@pytest.mark.parametrize("plan", [STAGE, RING, FUSED, PAIR])
 def test_parity_periodic_boundary(C, model, stencil, integ, plan):
     cfg, Z = make(model, 37, 50, stencil, integ, boundary=1)
     got = gpu_run(C, cfg, Z, 30, plan=plan)
@@ -158,7 +159,7 @@ def test_parity_periodic_boundary(C, model, stencil, integ, plan):
 
 
 @pytest.mark.parametrize("model", [KARMA, BOCF])
-@pytest.mark.parametrize("plan", [STAGE, RING, FUSED])
+@pytest.mark.parametrize("plan", [STAGE, RING, FUSED, PAIR])
 def test_parity_tanhfree_variant(C, model, plan):
     cfg, Z = make(model, 40, 33, LAP9X4, RK4, variant=1)
     got = gpu_run(C, cfg, Z, 50, plan=plan)
@@ -170,7 +171,7 @@ def test_parity_tanhfree_variant(C, model, plan):
 
 @pytest.mark.parametrize("model,stencil,nx,ny", [(FHN, LAP5, 3, 3), (FHN, LAP9X4, 5, 5), (KARMA, LAP9X4, 5, 64),
                                                  (BOCF, LAP5, 200, 3), (FHN, BOX9, 3, 17), (KARMA, LAP5, 33, 4)])
-@pytest.mark.parametrize("plan", [STAGE, RING, FUSED])
+@pytest.mark.parametrize("plan", [STAGE, RING, FUSED, PAIR])
 def test_parity_degenerate_sizes(C, model, stencil, nx, ny, plan):
     """Minimum sizes 2r+1 (every stencil arm reflects; the fused window folds the grid several
     times over) and thin strips."""
@@ -180,7 +181,7 @@ def test_parity_degenerate_sizes(C, model, stencil, nx, ny, plan):
     assert maxabs(got, ref) <= TOL_100
 
 
-@pytest.mark.parametrize("plan", [STAGE, RING, FUSED])
+@pytest.mark.parametrize("plan", [STAGE, RING, FUSED, PAIR])
 def test_batch_members_independent_of_position(C, plan):
     cfg, Z = make(KARMA, 48, 40, LAP5, RK4, batch=5, seed=3)
     def gpu_run_p(C, cfg, Z, n):
@@ -199,7 +200,8 @@ def test_batch_members_independent_of_position(C, plan):
 @pytest.mark.parametrize("model,integ,plan", [(FHN, EULER, STAGE), (FHN, RK4, STAGE), (KARMA, HEUN, STAGE),
                                               (FHN, EULER, RING), (BOCF, RK4, RING), (KARMA, HEUN, RING),
                                               (BOCF, RL, STAGE), (FHN, EULER, FUSED), (FHN, RK4, FUSED),
-                                              (KARMA, HEUN, FUSED), (BOCF, EULER, FUSED)])
+                                              (KARMA, HEUN, FUSED), (BOCF, EULER, FUSED),
+                                              (BOCF, RK4, PAIR), (FHN, EULER, PAIR), (KARMA, HEUN, PAIR)])
 def test_step_composition_and_determinism_bitwise(C, model, integ, plan):
     """step(a); step(b) == step(a+b), graph replay == direct launches, temporally blocked Euler ==
     single Euler steps, run-to-run identical."""
@@ -225,6 +227,32 @@ def test_fused_many_tiles_matches_stage_plan_and_oracle(C):
         assert np.array_equal(gpu_run(C, cfg, Z, 12, plan=RING), direct)
 
 
+@pytest.mark.parametrize("model,stencil,integ,bc", [(BOCF, LAP9X4, RK4, 0), (BOCF, LAP5, RK4, 1), (BOCF, BOX9, HEUN, 0),
+                                                    (BOCF, LAP9X4, EULER, 1), (FHN, LAP9X4, RK4, 0), (KARMA, BOX9, RK4, 1),
+                                                    (KARMA, LAP5, HEUN, 0), (FHN, LAP5, EULER, 0)])
+def test_pair_plan_many_tiles_bitwise_equal_to_stage_plan(C, model, stencil, integ, bc):
+    """4 x 8 tiles of 64 x 24 cells with ragged edges (odd width), interior tiles (branch-free, 128-bit
+    path) and rim tiles (ghost cells evaluated at their images): the ring cells a tile recomputes for
+    its neighbours, and the combinations of the two fused substeps, are the stage plan's arithmetic —
+    the same bits; an odd number of Euler steps ends with one stage launch."""
+    cfg, Z = make(model, 251, 170, stencil, integ, seed=21, boundary=bc, batch=2)
+    got = gpu_run(C, cfg, Z, 13, plan=PAIR)
+    ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 13)
+    assert maxabs(got, ref) <= TOL_100
+    assert np.array_equal(got, gpu_run(C, cfg, Z, 13, plan=STAGE))
+
+
+def test_pair_plan_limits(C):
+    cfg, _ = make(BOCF, 40, 40, LAP5, RL)
+    with C.Context.from_config(cfg) as ctx:
+        with pytest.raises(C.CardiacError):
+            C.cardiac_set_plan(ctx.ctx, PAIR, 0)              # gate integrators: plan STAGE only
+    cfg, _ = make(BOCF, 40, 40, LAP5, RK4)
+    with C.Context.from_config(cfg) as ctx:
+        with pytest.raises(C.CardiacError):
+            C.cardiac_set_plan(ctx.ctx, PAIR, 3)
+
+
 def test_plan_switch_keeps_state(C):
     cfg, Z = make(FHN, 70, 45, LAP9X4, RK4)
     with C.Context.from_config(cfg, plan=FUSED) as ctx:
@@ -234,8 +262,16 @@ def test_plan_switch_keeps_state(C):
         ctx.step(4)
         C.cardiac_set_plan(ctx.ctx, FUSED, 0)
         ctx.step(2)
+        C.cardiac_set_plan(ctx.ctx, PAIR, 0)          # rotates the state through three buffers
+        ctx.step(2)
+        C.cardiac_set_plan(ctx.ctx, FUSED, 0)
+        ctx.step(1)
+        C.cardiac_set_plan(ctx.ctx, PAIR, 0)
+        ctx.step(2)
+        C.cardiac_set_plan(ctx.ctx, *STAGE)
+        ctx.step(1)
         got = ctx.get_state()
-    assert maxabs(got, O.step(FHN, Z, cfg.dx, cfg.dt, cfg.scheme, 9)) <= TOL_100
+    assert maxabs(got, O.step(FHN, Z, cfg.dx, cfg.dt, cfg.scheme, 15)) <= TOL_100
 
 
 def test_uniform_state_and_rest_state(C):

@@ -259,6 +259,53 @@ def run_sweep(args):
     print(json.dumps({"sweep": rows, "integrator": "rk4", "peak_gbs": peak}))
 
 
+def run_slabs(args, cfg):
+    """`--decompose slabs`: ONE grid of the config cut into row slabs over the ranks (strong scaling;
+    DESIGN.md "Multi-GPU", paper_1309_1720_b200/dist.py): every rank advances its slab plus ghost rows
+    with the single-GPU kernels and swaps r x substeps x k ghost rows with its neighbours every k time
+    steps (NCCL send/recv).  Not the default bench line: the BASELINE configs fit one GPU."""
+    import torch
+    rank, local_rank, world = D.env_world()
+    D.init("nccl")
+    torch.cuda.set_device(local_rank)
+    from paper_1309_1720_b200 import cardiac as C
+    stages = {W.EULER: 1, W.HEUN: 2, W.RK4: 4}.get(cfg.integrator, 1)
+    every = max(1, args.exchange_every)
+    g = D.ghost_depth(2 if cfg.stencil == W.LAP9X4 else 1, stages, every)
+    slab = D.slab_of(cfg.ny, rank, world, g, bool(cfg.boundary))
+    Z0 = np.ascontiguousarray(W.initial_state(cfg)[:, :, slab.global_rows(), :])
+    alloc = lambda n: torch.empty((cfg.batch, cfg.n_v, n, cfg.nx), dtype=torch.float64, device="cuda")
+    with C.Context(cfg.model, cfg.nx, slab.ext_rows, cfg.dx, cfg.dt, cfg.scheme, cfg.batch,
+                   plan=args.plan, plan_param=args.plan_param) as ctx:
+        ctx.set_state(Z0)
+        exchange = lambda: D.exchange_dist(ctx, slab, alloc)
+        for _ in range(args.warmup):
+            D.advance_slab(ctx, slab, cfg.nsteps, every, exchange)
+            exchange()
+        torch.cuda.synchronize(); D.barrier()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = ctx.launches
+        a.record()
+        for _ in range(args.steps):
+            D.advance_slab(ctx, slab, cfg.nsteps, every, exchange)
+            exchange()                          # the next run starts from fresh ghosts
+        b.record()
+        torch.cuda.synchronize(); D.barrier()
+        ms = D.max_over_ranks(a.elapsed_time(b))
+        launches = ctx.launches - l0
+        own = ctx.get_rows(slab.g_lo, slab.own)
+    if not np.all(np.isfinite(own)):
+        raise RuntimeError("non-finite state after the timed run")
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": cfg.cells * cfg.nsteps * args.steps / (ms * 1e-3) / 1e9, "unit": UNIT,
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+            "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.describe(), "parallelism": f"row slabs x{world}, {g} ghost rows per cut, "
+                       f"one exchange per {every} time step(s)", "rows_per_rank": slab.own},
+            "gpu_launches": int(launches)}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -271,6 +318,9 @@ def main():
     ap.add_argument("--nsteps", type=int, default=0, help="override the config's time steps per run (profiling only)")
     ap.add_argument("--no-extras", action="store_true", help="skip cpu_baseline, e2e and the other configs")
     ap.add_argument("--sweep", action="store_true", help="size sweep S of SURVEY.md 8(d) instead of the bench line")
+    ap.add_argument("--decompose", default="replicas", choices=["replicas", "slabs"],
+                    help="N > 1: independent replicas (default, weak scaling) or ONE grid in row slabs (strong)")
+    ap.add_argument("--exchange-every", type=int, default=1, help="slabs: time steps between ghost exchanges")
     args = ap.parse_args()
     if args.warmup < 3 and not args.no_extras:
         args.warmup = 3                         # timing rule: W >= 3
@@ -292,6 +342,9 @@ def main():
     import torch
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (the product has no CPU fallback)")
+    if args.decompose == "slabs":
+        run_slabs(args, cfg)
+        return
     D.init("nccl")
     torch.cuda.set_device(local_rank)
     from paper_1309_1720_b200 import cardiac as C

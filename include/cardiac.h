@@ -164,6 +164,23 @@ int cardiac_get_state(cardiac_ctx*, double* dst, int dst_on_device);
  * J_b = (phi(x + eps v_b) - phi(x)) / eps as dense [batch-1][n_v][ny][nx] float64 into dst. */
 int cardiac_get_jvp(cardiac_ctx*, double eps, double* dst, int dst_on_device);
 
+/* Row-slab decomposition of ONE grid across GPUs (the paper is single-GPU,
+ * PAPER.md:122).  A rank holds a context over its rows PLUS g ghost rows towards each neighbour, with
+ * g = radius x substeps per time step x time steps between exchanges: information travels one stencil
+ * radius per substep, so after those time steps the rank's own rows are exactly the
+ * single-grid result and only the ghost rows are stale.  The exchange reads the g own rows next to the
+ * cut and writes them into the neighbour's ghost rows with these two calls:
+ *   cardiac_get_rows  rows [j0, j0+nrows) of every field of every batch member -> dense
+ *                     [batch][n_v][nrows][nx] float64 at dst.  A DEVICE dst may be any address the
+ *                     GPU can store to, including peer memory mapped over NVLink (the pack kernel
+ *                     then is the transfer); asynchronous on the context stream.
+ *   cardiac_set_rows  the reverse.
+ * For 3-D contexts a "row" is an index of the flattened (plane, row) pair, so a slab of planes is a
+ * row range too.  Host buffers synchronise the stream.  CARDIAC_ERR_INVALID when the range leaves
+ * the grid, CARDIAC_ERR_NOSTATE before set_state. */
+int cardiac_get_rows(cardiac_ctx*, int j0, int nrows, double* dst, int dst_on_device);
+int cardiac_set_rows(cardiac_ctx*, int j0, int nrows, const double* src, int src_on_device);
+
 /* Diagnostic (not on the hot path): evaluate device-side building blocks on n sample points held
  * in device memory, enqueued on the context stream.
  *   CARDIAC_PROBE_EXP      out[i] = the library's exp(in[i])            (used inside tanh)

@@ -33,7 +33,8 @@ EXPORTS = [
     "cardiac_num_fields", "cardiac_num_params", "cardiac_default_params", "cardiac_create",
     "cardiac_set_params", "cardiac_get_params", "cardiac_set_stream", "cardiac_set_plan",
     "cardiac_get_plan", "cardiac_workspace_bytes", "cardiac_bind_workspace", "cardiac_set_state",
-    "cardiac_step", "cardiac_get_state", "cardiac_get_jvp", "cardiac_probe", "cardiac_launch_count",
+    "cardiac_step", "cardiac_get_state", "cardiac_get_jvp", "cardiac_get_rows", "cardiac_set_rows",
+    "cardiac_probe", "cardiac_launch_count",
     "cardiac_time_steps", "cardiac_last_error", "cardiac_destroy",
 ]
 
@@ -67,6 +68,8 @@ _sig = {
     "cardiac_step": (_i, [_vp, _ll]),
     "cardiac_get_state": (_i, [_vp, _vp, _i]),
     "cardiac_get_jvp": (_i, [_vp, _d, _vp, _i]),
+    "cardiac_get_rows": (_i, [_vp, _i, _i, _vp, _i]),
+    "cardiac_set_rows": (_i, [_vp, _i, _i, _vp, _i]),
     "cardiac_probe": (_i, [_vp, _i, _vp, _vp, _ll]),
     "cardiac_launch_count": (_ll, [_vp]),
     "cardiac_time_steps": (_i, [_vp, _ll, _i, ctypes.POINTER(ctypes.c_float)]),
@@ -181,6 +184,16 @@ def cardiac_get_jvp(ctx, eps: float, dst) -> None:
     _check(ctx, _lib.cardiac_get_jvp(ctx, eps, addr, dev))
 
 
+def cardiac_get_rows(ctx, j0: int, nrows: int, dst) -> None:
+    addr, dev, _keep = _buffer(dst)
+    _check(ctx, _lib.cardiac_get_rows(ctx, j0, nrows, addr, dev))
+
+
+def cardiac_set_rows(ctx, j0: int, nrows: int, src) -> None:
+    addr, dev, _keep = _buffer(src)
+    _check(ctx, _lib.cardiac_set_rows(ctx, j0, nrows, addr, dev))
+
+
 def cardiac_probe(ctx, what: int, src, dst, n: int) -> None:
     a, da, _k1 = _buffer(src)
     b, db, _k2 = _buffer(dst)
@@ -250,6 +263,16 @@ class Context:
             dst = np.empty(self.shape, dtype=np.float64)
         cardiac_get_state(self.ctx, dst)
         return dst
+
+    def get_rows(self, j0, nrows, dst=None):
+        """Rows [j0, j0+nrows) of every field and member as dense [batch][n_v][nrows][nx]."""
+        if dst is None:
+            dst = np.empty(self.shape[:2] + (nrows, self.shape[-1]), dtype=np.float64)
+        cardiac_get_rows(self.ctx, j0, nrows, dst)
+        return dst
+
+    def set_rows(self, j0, src):
+        cardiac_set_rows(self.ctx, j0, src.shape[-2], src)
 
     def get_jvp(self, eps, dst=None):
         if dst is None:

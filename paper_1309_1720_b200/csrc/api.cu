@@ -581,6 +581,45 @@ int cardiac_get_jvp(cardiac_ctx* c, double eps, double* dst, int dst_on_device) 
   return CARDIAC_OK;
 }
 
+namespace {
+int rows_copy(cardiac_ctx* c, int j0, int nrows, double* buf, int on_device, bool pack) {
+  if (!c) return CARDIAC_ERR_INVALID;
+  if (!buf) return fail(c, CARDIAC_ERR_INVALID, "null buffer");
+  if (!c->has_state) return fail(c, CARDIAC_ERR_NOSTATE, "no state set");
+  const Problem& pb = c->pb;
+  if (j0 < 0 || nrows < 0 || (long long)j0 + nrows > (long long)pb.ny * pb.nz)
+    return fail(c, CARDIAC_ERR_INVALID, "row range outside the grid");
+  if (nrows == 0) return CARDIAC_OK;
+  DeviceGuard guard(c->device);
+  if (on_device) {
+    cudaError_t e = launch_rows(pb, c->buf[c->cur], j0, nrows, buf, pack, c->stream);
+    if (e != cudaSuccess) return fail_cuda(c, e, "rows launch");
+    c->launches++;
+    return CARDIAC_OK;
+  }
+  const size_t bytes = (size_t)pb.batch * pb.nv * nrows * pb.nx * sizeof(double);
+  double* tmp = nullptr;
+  CK(cudaMalloc(&tmp, bytes));
+  cudaError_t e = cudaSuccess;
+  if (!pack) e = cudaMemcpyAsync(tmp, buf, bytes, cudaMemcpyHostToDevice, c->stream);
+  if (e == cudaSuccess) e = launch_rows(pb, c->buf[c->cur], j0, nrows, tmp, pack, c->stream);
+  if (e == cudaSuccess && pack) e = cudaMemcpyAsync(buf, tmp, bytes, cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  cudaFree(tmp);
+  if (e != cudaSuccess) return fail_cuda(c, e, "rows copy");
+  c->launches++;
+  return CARDIAC_OK;
+}
+}  // namespace
+
+int cardiac_get_rows(cardiac_ctx* c, int j0, int nrows, double* dst, int dst_on_device) {
+  return rows_copy(c, j0, nrows, dst, dst_on_device, true);
+}
+
+int cardiac_set_rows(cardiac_ctx* c, int j0, int nrows, const double* src, int src_on_device) {
+  return rows_copy(c, j0, nrows, const_cast<double*>(src), src_on_device, false);
+}
+
 int cardiac_probe(cardiac_ctx* c, int what, const double* in_dev, double* out_dev, long long n) {
   if (!c) return CARDIAC_ERR_INVALID;
   if (!in_dev || !out_dev || n < 0) return fail(c, CARDIAC_ERR_INVALID, "bad probe arguments");

@@ -40,6 +40,11 @@ constexpr long long kRingMinCells = 1 << 20;  // AUTO: below this the persistent
 cudaError_t launch_jvp(const Problem& pb, const double* state, double eps, double* dst_dense,
                        cudaStream_t stream);
 
+// rows [j0, j0 + nrows) of the flattened (plane, row) index of every field and member: state -> dense
+// [batch][n_v][nrows][nx] (pack) or back
+cudaError_t launch_rows(const Problem& pb, double* state, int j0, int nrows, double* dense, bool pack,
+                        cudaStream_t stream);
+
 // tile_kernels_*.cu: plan FUSED — all substeps of one time step (ksteps = 1), or ksteps forward-Euler
 // steps, in one launch on overlapped tiles (tile.cuh).  in != out.
 constexpr int kEulerBlock = 4;  // Euler steps per launch when temporally blocked

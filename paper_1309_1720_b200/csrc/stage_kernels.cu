@@ -249,7 +249,33 @@ __global__ void jvp_kernel(const double* __restrict__ Z, double* __restrict__ J,
   J[(long long)(b - 1) * n + e] = (Z[b * bstride + src] - Z[src]) / eps;
 }
 
+// rows [j0, j0 + nrows) of every field of every member <-> dense [batch * n_v][nrows][nx]
+// (ghost-row exchange of a row-slab decomposition, include/cardiac.h cardiac_get_rows / _set_rows)
+template <bool PACK>
+__global__ void rows_kernel(double* __restrict__ Z, double* __restrict__ D, int nx, int nrows, int j0,
+                            int pitch, long long fstride, long long n) {
+  const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n) return;
+  const int i = (int)(e % nx);
+  const long long t = e / nx;
+  const int j = (int)(t % nrows);
+  const long long f = t / nrows;   // member * n_v + field
+  const long long z = f * fstride + (long long)(j0 + j) * pitch + i;
+  if (PACK) D[e] = Z[z];
+  else Z[z] = D[e];
+}
+
 }  // namespace
+
+cudaError_t launch_rows(const Problem& pb, double* state, int j0, int nrows, double* dense, bool pack,
+                        cudaStream_t stream) {
+  const long long n = (long long)pb.batch * pb.nv * nrows * pb.nx;
+  if (n == 0) return cudaSuccess;
+  const unsigned blocks = (unsigned)((n + 255) / 256);
+  if (pack) rows_kernel<true><<<blocks, 256, 0, stream>>>(state, dense, pb.nx, nrows, j0, pb.pitch, pb.fstride, n);
+  else rows_kernel<false><<<blocks, 256, 0, stream>>>(state, dense, pb.nx, nrows, j0, pb.pitch, pb.fstride, n);
+  return cudaGetLastError();
+}
 
 cudaError_t launch_stage(const Problem& pb, const StageLaunch& st, cudaStream_t stream) {
   // DIRECT vs RING (bitwise identical results).  Measured on B200 (profiles/, r1 v4): with 32 warps

@@ -1,4 +1,4 @@
-// tile.cuh — the on-chip tile engine behind plans FUSED and PERSISTENT.
+// tile.cuh — the on-chip tile engine behind plan FUSED.
 //
 // One CTA advances one tile of the grid through ALL substeps of a time step (or through several
 // Euler steps) without leaving the SM: the paper's lock-step, one global round trip per substep
@@ -49,14 +49,6 @@ struct TileArgs {
   double b_dt[4];  // running sum       = acc + b_dt[s] f   (acc starts at y)
   double lapw[MD::ND];
   typename MD::Params p;
-  // PERSISTENT plan only
-  double* bufA;
-  double* bufB;
-  unsigned* flags;     // per tile: number of completed time steps
-  unsigned* abort_flag;
-  long long nsteps;
-  int tiles_x, tiles_y;
-  unsigned step_base;  // time steps completed before this launch (flags are monotonic)
 };
 
 // index of the grid cell that the even (no-flux) or periodic extension maps `i` to; any i

@@ -56,8 +56,6 @@ void fill_tile_args(const Problem& pb, int stencil, TileArgs<MD>& a) {
   }
   MD::derive(pb.params, a.p);
   for (int q = 0; q < MD::ND; ++q) a.lapw[q] = a.p.D[q] * stencil_norm(stencil) / (pb.dx * pb.dx);
-  a.bufA = a.bufB = nullptr; a.flags = nullptr; a.abort_flag = nullptr;
-  a.nsteps = 0; a.tiles_x = a.tiles_y = 0; a.step_base = 0;
 }
 
 template <class MD, int STENCIL, int INTEG, int KSTEPS, bool SMALL = false>

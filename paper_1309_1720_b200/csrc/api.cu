@@ -98,12 +98,14 @@ int auto_plan(const Problem& pb) {
   if (pb.nz > 1) return CARDIAC_PLAN_STAGE;   // 3-D: the stage-synchronous plan only
   if (resident_preferred(pb)) return CARDIAC_PLAN_PERSISTENT;
   if (rk_like && pb.model != CARDIAC_BOCF) return CARDIAC_PLAN_FUSED;
-  // 4-field model, Heun / RK4: two substeps per launch once the grid gives every SM >= ~20 waves of
-  // tiles (measured on B200: 4096^2 +5 %, 8192^2 +11 % over STAGE; at 2048^2 the
-  // 6.2 waves of 64 x 24 tiles lose 5 % to the last partial wave)
-  if (pb.model == CARDIAC_BOCF && (pb.integrator == I_HEUN || pb.integrator == I_RK4) &&
-      (long long)pb.nx * pb.ny * pb.batch >= kPairMinCells)
-    return CARDIAC_PLAN_PAIR;
+  // 4-field model: two substeps per launch once the grid gives every SM enough tiles (measured on B200,
+  // RK4 2048^2 +4 %, 4096^2 +13 %, 8192^2 +19 % over STAGE, equal at 1536^2, behind
+  // below; Heun +2 % at 4096^2, behind at 2048^2)
+  if (pb.model == CARDIAC_BOCF) {
+    const long long cells = (long long)pb.nx * pb.ny * pb.batch;
+    if ((pb.integrator == I_RK4 && cells >= kPairMinCellsRK4) || (pb.integrator == I_HEUN && cells >= kPairMinCellsHeun))
+      return CARDIAC_PLAN_PAIR;
+  }
   return CARDIAC_PLAN_STAGE;
 }
 

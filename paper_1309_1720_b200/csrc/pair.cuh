@@ -74,7 +74,14 @@ struct PairShape {
 // PRE (substep B = K_RK4F, tile cells): also forms the part of the final combination that does not
 // depend on substep B's result, P = w_B Y3 + (w_A Y2 + w_y y) — Y3 is this substep's input — and
 // stores it where substep B will write (which may be where Y2 was read: same thread, same cell).
-template <class MD, int STENCIL, int KIND, bool FULL, bool PRE>
+// a 128-bit global load the compiler may not sink towards its use
+CARDIAC_D double2 ld2v(const double* p) {
+  double2 v;
+  asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+  return v;
+}
+
+template <class MD, int STENCIL, int KIND, bool FULL, bool PRE, bool EARLY = false>
 CARDIAC_D void pair_from_global(const PairArgs<MD>& a, const double* __restrict__ in,
                                 const double* __restrict__ yb, const double* Ab, double* ob, int row, int x,
                                 double2 (&res)[MD::NV]) {
@@ -94,6 +101,16 @@ CARDIAC_D void pair_from_global(const PairArgs<MD>& a, const double* __restrict_
   double s0[ND], s1[ND];
 #pragma unroll
   for (int q = 0; q < ND; ++q) stencil_pair<STENCIL>(in + q * a.g.fstride, row, x, a.g.pitch, zz[q], s0[q], s1[q]);
+  // EARLY (tile cells of interior tiles): every global operand of the row is requested before the
+  // reaction starts, so that a warp waits for memory once per row; costs 8 registers per operand
+  double2 yy[NV], AA[NV];
+  if (EARLY) {
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) {
+      if (KIND != K_SELF) yy[q] = ld2v(yb + o + q * a.g.fstride);
+      if (PRE) AA[q] = ld2v(Ab + o + q * a.g.fstride);
+    }
+  }
   double z0[NV], z1[NV], f0[NV], f1[NV];
 #pragma unroll
   for (int q = 0; q < NV; ++q) { z0[q] = zz[q].x; z1[q] = zz[q].y; }
@@ -106,14 +123,16 @@ CARDIAC_D void pair_from_global(const PairArgs<MD>& a, const double* __restrict_
   }
 #pragma unroll
   for (int q = 0; q < NQ; ++q) {
-    double2 yy = make_double2(0.0, 0.0);
-    if (KIND != K_SELF) yy = ld2(yb + o + q * a.g.fstride);
-    res[q].x = combine<KIND>(a.a_wy, a.a_win, 0.0, 0.0, a.a_wf, yy.x, z0[q], 0.0, 0.0, f0[q]);
-    res[q].y = combine<KIND>(a.a_wy, a.a_win, 0.0, 0.0, a.a_wf, yy.y, z1[q], 0.0, 0.0, f1[q]);
+    if (!EARLY) {
+      yy[q] = make_double2(0.0, 0.0);
+      if (KIND != K_SELF) yy[q] = ld2(yb + o + q * a.g.fstride);
+      if (PRE) AA[q] = ld2(Ab + o + q * a.g.fstride);
+    }
+    res[q].x = combine<KIND>(a.a_wy, a.a_win, 0.0, 0.0, a.a_wf, yy[q].x, z0[q], 0.0, 0.0, f0[q]);
+    res[q].y = combine<KIND>(a.a_wy, a.a_win, 0.0, 0.0, a.a_wf, yy[q].y, z1[q], 0.0, 0.0, f1[q]);
     if (PRE) {
-      const double2 AA = ld2(Ab + o + q * a.g.fstride);
-      st2(ob + o + q * a.g.fstride, fma(a.w_B, z0[q], fma(a.w_A, AA.x, a.w_y * yy.x)),
-          fma(a.w_B, z1[q], fma(a.w_A, AA.y, a.w_y * yy.y)));
+      st2(ob + o + q * a.g.fstride, fma(a.w_B, z0[q], fma(a.w_A, AA[q].x, a.w_y * yy[q].x)),
+          fma(a.w_B, z1[q], fma(a.w_A, AA[q].y, a.w_y * yy[q].y)));
     }
   }
 }
@@ -254,8 +273,17 @@ __global__ void __launch_bounds__(PG::NT, PG::MINB)
 #pragma unroll 1
       for (int py = py0; py < TH; py += RSTEP) {   // tile cells: every field
         const int row = (y0 + py) * pitch;
+        if (py + RSTEP < TH) {   // the operands of this thread's next row: towards L1 while this row computes
+          const int on = row + RSTEP * pitch + x;
+#pragma unroll
+          for (int q = 0; q < NV; ++q) {
+            prefetch_l1(in + on + q * a.g.fstride);
+            if (KA == K_BASE) prefetch_l1(yb + on + q * a.g.fstride);
+            if (PRE) prefetch_l1(Ab + on + q * a.g.fstride);
+          }
+        }
         double2 res[NV];
-        pair_from_global<MD, STENCIL, KA, true, PRE>(a, in, yb, Ab, ob, row, x, res);
+        pair_from_global<MD, STENCIL, KA, true, PRE, true>(a, in, yb, Ab, ob, row, x, res);
 #pragma unroll
         for (int q = 0; q < NV; ++q) {
           if (q < ND) *reinterpret_cast<double2*>(sw + q * WSZ + (py + R) * WW + HX + 2 * px) = res[q];
@@ -296,9 +324,13 @@ __global__ void __launch_bounds__(PG::NT, PG::MINB)
 #pragma unroll 1
   for (int py = py0; py < rows; py += RSTEP) {
     const int o = (y0 + py) * pitch;
-    if (KB != K_SELF) {
+    double2 yq[NV];
+    if (KB != K_SELF) {   // this row's operand now (used after the reaction), the next row's towards L1
 #pragma unroll
-      for (int q = 0; q < NV; ++q) prefetch_l1(pb + o + q * a.g.fstride);
+      for (int q = 0; q < NV; ++q) {
+        if (py + RSTEP < rows) prefetch_l1(pb + o + RSTEP * pitch + q * a.g.fstride);
+        yq[q] = ld2v(pb + o + q * a.g.fstride);
+      }
     }
     const int srow = (py + R) * WW, sx = HX + 2 * px;
     double2 zz[NV];
@@ -320,8 +352,7 @@ __global__ void __launch_bounds__(PG::NT, PG::MINB)
     }
 #pragma unroll
     for (int q = 0; q < NV; ++q) {
-      double2 yy = make_double2(0.0, 0.0);
-      if (KB != K_SELF) yy = ld2(pb + o + q * a.g.fstride);
+      const double2 yy = KB != K_SELF ? yq[q] : make_double2(0.0, 0.0);
       double r0, r1;
       if (PRE) {   // = combine<K_RK4F> with its inner part already formed
         r0 = fma(a.w_f, f0[q], fma(a.w_in, z0[q], yy.x));

@@ -5,11 +5,14 @@
 
 namespace cardiac {
 
-// Tile: 64 x 24 cells, 256 threads (a thread keeps its column pair and walks 3 rows), three CTAs per SM at
-// 80 registers.  Shared memory per CTA = 8 B x (n_d x 68 x (24+2r) + (n_v-n_d) x 64 x 24): 52 KB for
-// BOCF with r = 2.  Measured on B200 against 64x16 / 64x24 at 64 registers (4 CTAs, spills in the row
-// loops) and 64x32 at 80 registers: 2048^2 BOCF LAP9X4 RK4 335 us per step against 367 / 415 / 368.
-using PairTile = PairGeom<64, 24, 256, 3>;
+// Tile: 64 x 24 cells, 256 threads (a thread keeps its column pair and walks 3 rows), TWO CTAs per SM at
+// 128 registers: the interior path requests every global operand of a row before the reaction starts
+// (one exposed memory latency per row instead of three), which needs the registers.  Shared memory per
+// CTA = 8 B x (n_d x 68 x (24+2r) + (n_v-n_d) x 64 x 24): 52 KB for BOCF with r = 2.  Measured on B200,
+// 2048^2 / 4096^2 BOCF LAP9X4 RK4, us per step: 310 / 1054; without the early loads 341 / 1188; three
+// CTAs at 80 registers 335 / 1126; four at 64 registers (spills in the row loops) 415 / 1365; register
+// double-buffering of the next row's stencil inputs 319 / 1115 (not kept).
+using PairTile = PairGeom<64, 24, 256, 2>;
 
 template <class MD, int STENCIL, int KA, int KB, bool STORE_MID>
 cudaError_t pair_run(const Problem& pb, const PairLaunch& pl, cudaStream_t stream) {

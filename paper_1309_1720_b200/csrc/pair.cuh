@@ -259,6 +259,10 @@ __global__ void __launch_bounds__(PG::NT, PG::MINB)
   const long long base = (long long)blockIdx.z * a.g.bstride;
   const int tid = threadIdx.x;
   const int py0 = tid / PW, px = tid - py0 * PW;   // a thread keeps its column pair; rows py0, py0 + RSTEP, ...
+  // programmatic dependent launch: this grid may be scheduled while the previous launch drains; every
+  // global access below waits for that grid to complete and flush
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
   // ---------------------------------------------------------------- phase 1: substep A -> shared memory
   // block-uniform: the window and the stencil arms of its outermost cells lie inside the grid

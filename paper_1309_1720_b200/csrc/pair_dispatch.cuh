@@ -38,8 +38,17 @@ cudaError_t pair_run(const Problem& pb, const PairLaunch& pl, cudaStream_t strea
   MD::derive(pb.params, a.p);
   for (int q = 0; q < MD::ND; ++q) a.lapw[q] = a.p.D[q] * stencil_norm(STENCIL) / (pb.dx * pb.dx);
   dim3 grid((pb.nx + PG::TW - 1) / PG::TW, (pb.ny + PG::TH - 1) / PG::TH, pb.batch);
-  kern<<<grid, PG::NT, S::SMEM_BYTES, stream>>>(a);
-  return cudaGetLastError();
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = dim3(PG::NT);
+  cfg.dynamicSmemBytes = S::SMEM_BYTES;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, a);
 }
 
 template <class MD, int STENCIL>

@@ -69,11 +69,6 @@ struct PairShape {
   static_assert(TW % 2 == 0 && R <= HX, "");
 };
 
-// Substep KIND of the x-adjacent pair at (x, row/pitch), every operand from global memory, no boundary
-// logic.  FULL: all fields; otherwise the diffusing fields only (the rest of the reaction is dead code).
-// PRE (substep B = K_RK4F, tile cells): also forms the part of the final combination that does not
-// depend on substep B's result, P = w_B Y3 + (w_A Y2 + w_y y) — Y3 is this substep's input — and
-// stores it where substep B will write (which may be where Y2 was read: same thread, same cell).
 // a 128-bit global load the compiler may not sink towards its use
 CARDIAC_D double2 ld2v(const double* p) {
   double2 v;
@@ -81,6 +76,11 @@ CARDIAC_D double2 ld2v(const double* p) {
   return v;
 }
 
+// Substep KIND of the x-adjacent pair at (x, row/pitch), every operand from global memory, no boundary
+// logic.  FULL: all fields; otherwise the diffusing fields only (the rest of the reaction is dead code).
+// PRE (substep B = K_RK4F, tile cells): also forms the part of the final combination that does not
+// depend on substep B's result, P = w_B Y3 + (w_A Y2 + w_y y) — Y3 is this substep's input — and
+// stores it where substep B will write (which may be where Y2 was read: same thread, same cell).
 template <class MD, int STENCIL, int KIND, bool FULL, bool PRE, bool EARLY = false>
 CARDIAC_D void pair_from_global(const PairArgs<MD>& a, const double* __restrict__ in,
                                 const double* __restrict__ yb, const double* Ab, double* ob, int row, int x,

@@ -251,6 +251,22 @@ def test_pair_plan_limits(C):
     with C.Context.from_config(cfg) as ctx:
         with pytest.raises(C.CardiacError):
             C.cardiac_set_plan(ctx.ctx, PAIR, 3)
+    # AUTO: the 4-field model with RK4 from 4 Mi cells (config 4), Heun from 12 Mi; STAGE below
+    for n, integ, want in [(2048, RK4, PAIR), (1536, RK4, 1), (2048, HEUN, 1), (3584, HEUN, PAIR), (2048, EULER, 1)]:
+        ctx = C.cardiac_create(BOCF, n, n, 0.03, 0.09, LAP9X4 | integ_bits(C, integ), 1)
+        try:
+            assert C.cardiac_get_plan(ctx) == want, (n, integ)
+        finally:
+            C.cardiac_destroy(ctx)
+    ctx = C.cardiac_create(FHN, 2048, 2048, 0.04, 1e-4, C.CARDIAC_LAP9X4 | C.CARDIAC_RK4, 1)
+    try:
+        assert C.cardiac_get_plan(ctx) == FUSED
+    finally:
+        C.cardiac_destroy(ctx)
+
+
+def integ_bits(C, integ):
+    return {EULER: C.CARDIAC_EULER, HEUN: C.CARDIAC_HEUN, RK4: C.CARDIAC_RK4}[integ]
 
 
 def test_plan_switch_keeps_state(C):

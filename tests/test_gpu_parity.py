@@ -242,6 +242,19 @@ def test_pair_plan_many_tiles_bitwise_equal_to_stage_plan(C, model, stencil, int
     assert np.array_equal(got, gpu_run(C, cfg, Z, 13, plan=STAGE))
 
 
+@pytest.mark.parametrize("nx,ny", [(64, 24), (65, 25), (66, 26), (67, 23), (68, 48), (69, 47), (128, 49), (130, 72),
+                                   (63, 22), (5, 100), (200, 5), (132, 28)])
+@pytest.mark.parametrize("stencil,bc", [(LAP9X4, 0), (LAP9X4, 1), (BOX9, 0), (LAP5, 1)])
+def test_pair_plan_tile_edges(C, nx, ny, stencil, bc):
+    """Grid sizes around the 64 x 24 tile and its 4-cell / r-row margins: exactly one tile, one cell or one
+    pair more, ghost cells inside a ragged tile, tiles whose ring is entirely ghost cells, strips thinner
+    than a ring.  Bitwise the stage plan, and the oracle."""
+    cfg, Z = make(BOCF, nx, ny, stencil, RK4, seed=nx * 131 + ny, boundary=bc)
+    got = gpu_run(C, cfg, Z, 3, plan=PAIR)
+    assert np.array_equal(got, gpu_run(C, cfg, Z, 3, plan=STAGE))
+    assert maxabs(got, O.step(BOCF, Z, cfg.dx, cfg.dt, cfg.scheme, 3)) <= TOL_100
+
+
 def test_pair_plan_limits(C):
     cfg, _ = make(BOCF, 40, 40, LAP5, RL)
     with C.Context.from_config(cfg) as ctx:

@@ -86,10 +86,19 @@ void carve(cardiac_ctx* c) {
 int fused_window_auto(const Problem& pb) {
   if (pb.nv > 2 || pb.integrator == I_EULER) return 1;
   const int H = pb.radius * stages_of(pb.integrator);
-  if (H <= 4) return 2;
-  const long long tw = 48 - 2 * H, th = 40 - 2 * H;
-  const long long ctas = ((pb.nx + tw - 1) / tw) * ((pb.ny + th - 1) / th) * pb.batch;
-  return ctas <= 148 ? 2 : 1;
+  auto ctas = [&](long long ew, long long eh) {
+    const long long tw = ew - 2 * H, th = eh - 2 * H;
+    return ((pb.nx + tw - 1) / tw) * ((pb.ny + th - 1) / th) * pb.batch;
+  };
+  const long long small = ctas(48, 40), large = ctas(80, 48);
+  if (small <= 148) return 2;   // one small CTA per SM: the shortest CTA lifetime
+  if (H > 4) return 1;          // 40 % useful cells against 53 %
+  // H <= 4: both windows keep 3840 cells per SM busy; a wave of large CTAs (one per SM, lock step)
+  // takes 1.18 x a wave of small ones (two per SM, out of step: time grows linearly with the count,
+  // plus 0.57 of a wave of start-up).  Measured on B200, Karma LAP5 RK4 512^2 - 1536^2: the large window
+  // wins where its tiles fill whole waves (640^2: 10.8 against 15.6 us per step, 1280^2: 40.8 / 43.4)
+  const double waves_large = (double)((large + 147) / 148);
+  return waves_large * 1.18 < 0.57 + (double)small / 296.0 ? 1 : 2;
 }
 
 int auto_plan(const Problem& pb) {

@@ -92,7 +92,11 @@ int fused_window_auto(const Problem& pb) {
   };
   const long long small = ctas(48, 40), large = ctas(80, 48);
   if (small <= 148) return 2;   // one small CTA per SM: the shortest CTA lifetime
-  if (H > 4) return 1;          // 40 % useful cells against 53 %
+  if (H > 4) {                  // 40 % useful cells against 53 %: one CTA per SM, time = waves x window area
+    if (pb.integrator != I_RK4 || pb.radius != 2) return 1;
+    const long long tall = ctas(64, 56);
+    return ((tall + 147) / 148) * (64 * 56) < ((large + 147) / 148) * (80 * 48) ? 3 : 1;
+  }
   // H <= 4: both windows keep 3840 cells per SM busy; a wave of large CTAs (one per SM, lock step)
   // takes 1.18 x a wave of small ones (two per SM, out of step: time grows linearly with the count,
   // plus 0.57 of a wave of start-up).  Measured on B200, Karma LAP5 RK4 512^2 - 1536^2: the large window
@@ -118,15 +122,15 @@ int auto_plan(const Problem& pb) {
   return CARDIAC_PLAN_STAGE;
 }
 
-// FUSED + Heun/RK4: plan_param 1 = large window, 2 = small window (set_plan resolves 0)
-bool fused_small(const cardiac_ctx* c) {
-  return c->plan == CARDIAC_PLAN_FUSED && c->pb.integrator != I_EULER && c->plan_param == 2;
+// FUSED + Heun/RK4: plan_param = window (set_plan resolves 0)
+int fused_window(const cardiac_ctx* c) {
+  return (c->plan == CARDIAC_PLAN_FUSED && c->pb.integrator != I_EULER) ? c->plan_param : 1;
 }
 
 // Plan FUSED: one launch advances `ksteps` time steps (1, or kEulerBlock Euler steps), ping-pong.
 int enqueue_fused(cardiac_ctx* c, cudaStream_t s, int ksteps) {
   const int other = c->cur == 0 ? 1 : 0;   // (plan PAIR may have left the state in buffer 2)
-  TileLaunch tl{c->buf[c->cur], c->buf[other], ksteps, fused_small(c)};
+  TileLaunch tl{c->buf[c->cur], c->buf[other], ksteps, fused_window(c)};
   cudaError_t e = launch_fused(c->pb, tl, s);
   if (e != cudaSuccess) return fail_cuda(c, e, "fused launch");
   c->launches++;
@@ -447,9 +451,11 @@ int cardiac_set_plan(cardiac_ctx* c, int plan, int param) {
       if (rparam != 1 && rparam != kEulerBlock)
         return fail(c, CARDIAC_ERR_INVALID, "FUSED + Euler: steps per launch must be 1 or 4");
     } else {
-      if (param < 0 || param > 2 || (param == 2 && c->pb.nv > 2))
+      if (param < 0 || param > 3 || (param >= 2 && c->pb.nv > 2) ||
+          (param == 3 && (integ != I_RK4 || c->pb.radius != 2)))
         return fail(c, CARDIAC_ERR_INVALID,
-                    "FUSED + Heun/RK4: parameter 0 (auto), 1 (80x48 window) or 2 (48x40 window, 2-field models)");
+                    "FUSED + Heun/RK4: parameter 0 (auto), 1 (80x48 window), 2 (48x40 window, 2-field models) "
+                    "or 3 (64x56 window, 2-field models, RK4, 4th-order stencil)");
       rparam = param == 0 ? fused_window_auto(c->pb) : param;
     }
   } else if (resolved == CARDIAC_PLAN_PAIR) {

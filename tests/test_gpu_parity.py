@@ -91,6 +91,13 @@ def test_parity_fused_small_window(C, model, stencil, integ):
     assert maxabs(small, large) <= 1e-12
     auto = gpu_run(C, cfg, Z, 40, plan=(2, 0))
     assert np.array_equal(auto, small) or np.array_equal(auto, large)
+    if stencil == LAP9X4 and integ == RK4:          # the 64 x 56 window (halo 8: tile 48 x 40), 4 x 3 ragged tiles
+        tall = gpu_run(C, cfg, Z, 40, plan=(2, 3))
+        assert maxabs(tall, ref) <= TOL_100 and maxabs(tall, large) <= 1e-12
+    else:
+        with C.Context.from_config(cfg, plan=2) as ctx:
+            with pytest.raises(C.CardiacError):
+                C.cardiac_set_plan(ctx.ctx, 2, 3)
     with C.Context.from_config(W.make_config("b", BOCF, 64, LAP5, RK4, 0), plan=2) as ctx:
         with pytest.raises(C.CardiacError):
             C.cardiac_set_plan(ctx.ctx, 2, 2)          # the 4-field model has one window only

@@ -131,7 +131,7 @@ int cardiac_set_stream(cardiac_ctx*, void* cuda_stream);
 /* Choose the execution plan (CARDIAC_PLAN_*).  CARDIAC_ERR_INVALID if the plan does not support
  * the context's (model, scheme, size). `param` is plan specific: FUSED + Euler = time steps per
  * launch (0 = default); FUSED + Heun/RK4 = window (0 = by size, 1 = 80x48 cells, one CTA per SM,
- * 2 = 48x40 cells, two CTAs per SM, two-field models only, 3 = 64x56 cells, two-field models with RK4 and the 4th-order stencil); STAGE = kernel implementation (0 = by size, 1 = DIRECT: every thread loads
+ * 2 = 48x40 cells, two CTAs per SM, two-field models only, 3 / 4 / 5 = 64x56 / 64x48 / 56x48 cells, two-field models with RK4); STAGE = kernel implementation (0 = by size, 1 = DIRECT: every thread loads
  * its own operands, 2 = RING: persistent CTAs fed by a TMA shared-memory ring; same results
  * bitwise); PAIR, PERSISTENT: 0.  AUTO: PERSISTENT below ~100x100 cells per member, FUSED for the
  * two-field models, PAIR for the four-field model with RK4 from 4 Mi cells (Heun: 12 Mi), else STAGE. */

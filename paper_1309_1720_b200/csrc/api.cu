@@ -78,11 +78,17 @@ void carve(cardiac_ctx* c) {
 // round trip per substep dominates (FHN, Karma); the 4-field ionic model is FP64-pipe bound and its
 // register-resident patches are too small to amortise an 8-cell halo, so it stays stage-synchronous
 // (DESIGN.md "Plans").
-// FUSED + Heun/RK4: which window.  1 = large (80 x 48, one CTA per SM), 2 = small (48 x 40, two CTAs
-// per SM; two-field models).  Measured on B200: with a halo of H <= 4 cells the two
-// co-resident CTAs hide each other's load and barrier phases and the small window wins at every size
-// (Karma LAP5 RK4 2048^2: 30.9 -> 36.8 Gcell-step/s); with H = 8 its 40 % useful cells lose against
-// 53 % unless the whole grid is one wave of small tiles (<= 256^2: 7.7 -> 6.3 us per step).
+// FUSED + Heun/RK4: which window.  1 = 80 x 48 cells, 3 = 64 x 56, 4 = 64 x 48, 5 = 56 x 48 (one CTA per SM;
+// 3-5: RK4 of the two-field models), 2 = 48 x 40 (two CTAs per SM; two-field models).  Measured on B200
+// (Karma LAP5 RK4 and FHN LAP9X4 RK4, 362^2 - 1536^2, every window forced):
+//  * one CTA per SM: the CTAs of a wave run in lock step and a time step costs (waves) x (CTA lifetime),
+//    the lifetime being a fixed part (launch, window load, barriers, store) worth ~2000 cells plus the
+//    window area — 10.3 / 10.0 / 8.8 / 8.6 us per wave for windows 1 / 3 / 4 / 5 (Karma), 7.0 / 6.5 / 5.6 /
+//    5.4 us (FHN).  The window whose tiles fill whole waves wins: 512^2 with a halo of 8 is one wave of
+//    143 CTAs of window 3 (7.0 us) or of 128 of window 1 (7.4 us), but two waves of window 4 (11.1 us).
+//  * two small CTAs per SM run out of step: time grows linearly with their number n, 0.57 + n/296
+//    waves of 1/1.18 of window 1's wave time.  With a halo of 8 the small window has 40 % useful cells
+//    against 53 % and only wins when the whole grid is one CTA per SM (<= 256^2: 7.7 -> 6.3 us per step).
 int fused_window_auto(const Problem& pb) {
   if (pb.nv > 2 || pb.integrator == I_EULER) return 1;
   const int H = pb.radius * stages_of(pb.integrator);
@@ -90,19 +96,25 @@ int fused_window_auto(const Problem& pb) {
     const long long tw = ew - 2 * H, th = eh - 2 * H;
     return ((pb.nx + tw - 1) / tw) * ((pb.ny + th - 1) / th) * pb.batch;
   };
-  const long long small = ctas(48, 40), large = ctas(80, 48);
-  if (small <= 148) return 2;   // one small CTA per SM: the shortest CTA lifetime
-  if (H > 4) {                  // 40 % useful cells against 53 %: one CTA per SM, time = waves x window area
-    if (pb.integrator != I_RK4 || pb.radius != 2) return 1;
-    const long long tall = ctas(64, 56);
-    return ((tall + 147) / 148) * (64 * 56) < ((large + 147) / 148) * (80 * 48) ? 3 : 1;
+  const long long small = ctas(48, 40);
+  if (small <= 148) return 2;
+  constexpr double kFixed = 2000.0;   // cells
+  auto cost = [&](long long ew, long long eh) {
+    return (double)((ctas(ew, eh) + 147) / 148) * ((double)(ew * eh) + kFixed);
+  };
+  int best = 1;
+  double best_cost = cost(80, 48);
+  if (pb.integrator == I_RK4) {
+    const double c3 = cost(64, 56), c4 = cost(64, 48), c5 = cost(56, 48);
+    if (c3 < best_cost) { best = 3; best_cost = c3; }
+    if (c4 < best_cost) { best = 4; best_cost = c4; }
+    if (c5 < best_cost) { best = 5; best_cost = c5; }
   }
-  // H <= 4: both windows keep 3840 cells per SM busy; a wave of large CTAs (one per SM, lock step)
-  // takes 1.18 x a wave of small ones (two per SM, out of step: time grows linearly with the count,
-  // plus 0.57 of a wave of start-up).  Measured on B200, Karma LAP5 RK4 512^2 - 1536^2: the large window
-  // wins where its tiles fill whole waves (640^2: 10.8 against 15.6 us per step, 1280^2: 40.8 / 43.4)
-  const double waves_large = (double)((large + 147) / 148);
-  return waves_large * 1.18 < 0.57 + (double)small / 296.0 ? 1 : 2;
+  if (H <= 4) {
+    const double c2 = (80.0 * 48.0 + kFixed) / 1.18 * (0.57 + (double)small / 296.0);
+    if (c2 < best_cost) best = 2;
+  }
+  return best;
 }
 
 int auto_plan(const Problem& pb) {
@@ -451,11 +463,10 @@ int cardiac_set_plan(cardiac_ctx* c, int plan, int param) {
       if (rparam != 1 && rparam != kEulerBlock)
         return fail(c, CARDIAC_ERR_INVALID, "FUSED + Euler: steps per launch must be 1 or 4");
     } else {
-      if (param < 0 || param > 3 || (param >= 2 && c->pb.nv > 2) ||
-          (param == 3 && (integ != I_RK4 || c->pb.radius != 2)))
+      if (param < 0 || param > 5 || (param >= 2 && c->pb.nv > 2) || (param >= 3 && integ != I_RK4))
         return fail(c, CARDIAC_ERR_INVALID,
                     "FUSED + Heun/RK4: parameter 0 (auto), 1 (80x48 window), 2 (48x40 window, 2-field models) "
-                    "or 3 (64x56 window, 2-field models, RK4, 4th-order stencil)");
+                    "or 3 / 4 / 5 (64x56 / 64x48 / 56x48 window, 2-field models, RK4)");
       rparam = param == 0 ? fused_window_auto(c->pb) : param;
     }
   } else if (resolved == CARDIAC_PLAN_PAIR) {

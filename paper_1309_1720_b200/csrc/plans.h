@@ -52,7 +52,7 @@ struct TileLaunch {
   const double* in;
   double* out;
   int ksteps;
-  int window;  // Heun / RK4: 1 = 80 x 48 cells; two-field models also 2 = 48 x 40 (two CTAs per SM), 3 = 64 x 56 (RK4, radius 2)
+  int window;  // Heun / RK4: 1 = 80 x 48 cells; two-field models also 2 = 48 x 40 (two CTAs per SM) and, RK4, 3 / 4 / 5 = 64 x 56 / 64 x 48 / 56 x 48
 };
 cudaError_t launch_fused_fhn(const Problem& pb, const TileLaunch& tl, cudaStream_t stream);
 cudaError_t launch_fused_karma(const Problem& pb, const TileLaunch& tl, cudaStream_t stream);

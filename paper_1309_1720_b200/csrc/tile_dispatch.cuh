@@ -26,6 +26,15 @@ template <class MD, int H>
 struct FusedGeom<MD, H, 3> {
   using type = TileGeom<32, 14, 4>;
 };
+// two more one-CTA-per-SM windows for grids that the others tile into a badly filled last wave
+template <class MD, int H>
+struct FusedGeom<MD, H, 4> {
+  using type = TileGeom<32, 12, 4>;  // 64 x 48 window, 384 threads
+};
+template <class MD, int H>
+struct FusedGeom<MD, H, 5> {
+  using type = TileGeom<28, 12, 4>;  // 56 x 48 window, 336 threads
+};
 template <int VARIANT, int H, int WIN>
 struct FusedGeom<Model<M_BOCF, VARIANT>, H, WIN> {
   using type = TileGeom<24, 16, 2>;  // 48 x 32 window, 384 threads
@@ -99,8 +108,9 @@ cudaError_t fused_by_integrator(const Problem& pb, const TileLaunch& tl, cudaStr
     case I_RK4:
       if constexpr (MD::NV <= 2) {
         if (tl.window == 2) return fused_run<MD, STENCIL, I_RK4, 1, 2>(pb, tl, s);
-        if constexpr (STENCIL == S_LAP9X4)
-          if (tl.window == 3) return fused_run<MD, STENCIL, I_RK4, 1, 3>(pb, tl, s);
+        if (tl.window == 3) return fused_run<MD, STENCIL, I_RK4, 1, 3>(pb, tl, s);
+        if (tl.window == 4) return fused_run<MD, STENCIL, I_RK4, 1, 4>(pb, tl, s);
+        if (tl.window == 5) return fused_run<MD, STENCIL, I_RK4, 1, 5>(pb, tl, s);
       }
       return fused_run<MD, STENCIL, I_RK4, 1>(pb, tl, s);
     case I_HEUN:

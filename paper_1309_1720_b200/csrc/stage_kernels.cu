@@ -52,6 +52,19 @@ CARDIAC_D double zarm_edge(const double* __restrict__ U, int oc, int kz, int nz,
   return 0.0;
 }
 
+// One gate x' = alpha x + beta with the coefficients frozen at u^n, alpha < 0:
+// Rush-Larsen x+ = x_inf + (x - x_inf) e^{alpha dt}, x_inf = -beta/alpha; implicit Euler
+// x+ = (x + dt beta)/(1 - dt alpha).  The division is a reciprocal of a positive number (fastmath.cuh).
+template <int KIND>
+CARDIAC_D double gate_step(double dt, double x, double alpha, double beta) {
+  if (KIND == K_RL) {
+    const double e = exp_c(alpha * dt);
+    const double xinf = beta * rcp_pos(-alpha);
+    return fma(x - xinf, e, xinf);
+  }
+  return fma(dt, beta, x) * rcp_pos(fma(-dt, alpha, 1.0));
+}
+
 // the update of one cell once f = D lap + N is known; o = offset of the cell inside its field
 template <class MD, int KIND>
 CARDIAC_D void finish_cell(const StageArgs<MD>& a, const double* __restrict__ yb,
@@ -66,17 +79,7 @@ CARDIAC_D void finish_cell(const StageArgs<MD>& a, const double* __restrict__ yb
       MD::gates(a.p, z[0], alpha, beta);
       ob[o] = fma(a.dt, f[0], z[0]);
 #pragma unroll
-      for (int g = 0; g < 3; ++g) {
-        double x = z[g + 1], xn;
-        if (KIND == K_RL) {
-          double e = exp(alpha[g] * a.dt);
-          double xinf = -beta[g] / alpha[g];
-          xn = fma(x - xinf, e, xinf);
-        } else {
-          xn = fma(a.dt, beta[g], x) / fma(-a.dt, alpha[g], 1.0);
-        }
-        ob[o + (g + 1) * a.g.fstride] = xn;
-      }
+      for (int g = 0; g < 3; ++g) ob[o + (g + 1) * a.g.fstride] = gate_step<KIND>(a.dt, z[g + 1], alpha[g], beta[g]);
     }
     return;
   }
@@ -112,7 +115,7 @@ __global__ void __launch_bounds__(TX * TY, 8)
   // block-uniform: tile and halo inside the grid -> no boundary logic, 128-bit accesses
   const bool interior = x0 >= 2 && x0 + 2 * TX + 2 <= nx && j0 >= R && j0 + TY + R <= ny &&
                         (!D3 || (kz >= R && kz + R < a.g.nz));
-  if (interior && KIND != K_RL && KIND != K_IE) {
+  if (interior) {
     const int row = j * pitch;
     const off_t o = pz + row + x;
     // The gating fields are first used ~400 instructions into the reaction and y at its very end;
@@ -153,6 +156,19 @@ __global__ void __launch_bounds__(TX * TY, 8)
       f0[q] = fma(a.lapw[q], s0[q], f0[q]);
       f1[q] = fma(a.lapw[q], s1[q], f1[q]);
     }
+    if constexpr (KIND == K_RL || KIND == K_IE) {   // BOCF: u by Euler, the gates with frozen coefficients
+      if constexpr (NV == 4) {
+        double al0[3], be0[3], al1[3], be1[3];
+        MD::gates(a.p, z0[0], al0, be0);
+        MD::gates(a.p, z1[0], al1, be1);
+        st2(ob + o, fma(a.dt, f0[0], z0[0]), fma(a.dt, f1[0], z1[0]));
+#pragma unroll
+        for (int g = 0; g < 3; ++g)
+          st2(ob + o + (g + 1) * a.g.fstride, gate_step<KIND>(a.dt, z0[g + 1], al0[g], be0[g]),
+              gate_step<KIND>(a.dt, z1[g + 1], al1[g], be1[g]));
+      }
+      return;
+    }
 #pragma unroll
     for (int q = 0; q < NV; ++q) {
       double2 yy = make_double2(0.0, 0.0), AA = yy, BB = yy;
@@ -165,7 +181,7 @@ __global__ void __launch_bounds__(TX * TY, 8)
     return;
   }
 
-  // rim blocks (and the gate integrators): one cell at a time, boundary rule per neighbour
+  // rim blocks: one cell at a time, boundary rule per neighbour
   if (j >= ny) return;
   const int bc = a.g.boundary;
 #pragma unroll

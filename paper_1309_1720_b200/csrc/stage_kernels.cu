@@ -115,9 +115,11 @@ __global__ void __launch_bounds__(TX * TY, 8)
   // block-uniform: tile and halo inside the grid -> no boundary logic, 128-bit accesses
   const bool interior = x0 >= 2 && x0 + 2 * TX + 2 <= nx && j0 >= R && j0 + TY + R <= ny &&
                         (!D3 || (kz >= R && kz + R < a.g.nz));
+  const int row = j * pitch;
+  const off_t o = pz + row + x;
+  double2 zz[NV];
+  double s0[ND], s1[ND];
   if (interior) {
-    const int row = j * pitch;
-    const off_t o = pz + row + x;
     // The gating fields are first used ~400 instructions into the reaction and y at its very end;
     // under the 64-register cap ptxas sinks those loads next to their use (a second and third exposed
     // latency per warp).  Asking L1 for the lines now costs no register; the late loads then hit.
@@ -132,75 +134,111 @@ __global__ void __launch_bounds__(TX * TY, 8)
         for (int q = 0; q < NV; ++q) prefetch_l1(yb + o + q * a.g.fstride);
       }
     }
-    double2 zz[NV];
 #pragma unroll
     for (int q = 0; q < NV; ++q) zz[q] = ld2(in + o + q * a.g.fstride);
     // Stencil first: its neighbour loads go out together with the centre loads and are reduced to
     // two sums per diffusing field before the (register-hungry) reaction starts.  The RK operands
     // y / Y2 / Y3 are loaded after it, next to their use: with the kernel held to 64 registers
-    // (4 blocks = 32 warps per SM) the other warps cover that second latency, which measured faster
+    // (32 warps per SM) the other warps cover that second latency, which measured faster
     // than keeping 12 more 128-bit loads in flight per thread (or prefetching them to L1).
-    double s0[ND], s1[ND];
 #pragma unroll
     for (int q = 0; q < ND; ++q) {
       stencil_pair<STENCIL>(in + q * a.g.fstride + pz, row, x, pitch, zz[q], s0[q], s1[q]);
       if (D3) zarm_pair<STENCIL>(in + q * a.g.fstride, o, a.g.zstride, zz[q], s0[q], s1[q]);
     }
-    double z0[NV], z1[NV], f0[NV], f1[NV];
+  } else {
+    // rim blocks
+    if (j >= ny || x >= nx) return;
+    const int bc = a.g.boundary;
+    if (x + 1 >= nx) {   // the last cell of an odd row: alone, boundary rule per neighbour
+      const int oc = row + x;
+      double z[NV], f[NV];
 #pragma unroll
-    for (int q = 0; q < NV; ++q) { z0[q] = zz[q].x; z1[q] = zz[q].y; }
-    MD::reaction(a.p, z0, f0);
-    MD::reaction(a.p, z1, f1);
+      for (int q = 0; q < NV; ++q) z[q] = in[o + q * a.g.fstride];
+      MD::reaction(a.p, z, f);
 #pragma unroll
-    for (int q = 0; q < ND; ++q) {
-      f0[q] = fma(a.lapw[q], s0[q], f0[q]);
-      f1[q] = fma(a.lapw[q], s1[q], f1[q]);
-    }
-    if constexpr (KIND == K_RL || KIND == K_IE) {   // BOCF: u by Euler, the gates with frozen coefficients
-      if constexpr (NV == 4) {
-        double al0[3], be0[3], al1[3], be1[3];
-        MD::gates(a.p, z0[0], al0, be0);
-        MD::gates(a.p, z1[0], al1, be1);
-        st2(ob + o, fma(a.dt, f0[0], z0[0]), fma(a.dt, f1[0], z1[0]));
-#pragma unroll
-        for (int g = 0; g < 3; ++g)
-          st2(ob + o + (g + 1) * a.g.fstride, gate_step<KIND>(a.dt, z0[g + 1], al0[g], be0[g]),
-              gate_step<KIND>(a.dt, z1[g + 1], al1[g], be1[g]));
+      for (int q = 0; q < ND; ++q) {
+        double s = stencil_edge<STENCIL>(in + q * a.g.fstride + pz, x, j, nx, ny, pitch, bc, z[q]);
+        if (D3) s += zarm_edge<STENCIL>(in + q * a.g.fstride, oc, kz, a.g.nz, a.g.zstride, bc, z[q]);
+        f[q] = fma(a.lapw[q], s, f[q]);
       }
+      finish_cell<MD, KIND>(a, yb, Ab, Bb, ob, o, z, f);
       return;
     }
+    // A pair inside the grid whose stencil may reach across the boundary: the pair and its vertical
+    // (and z) neighbours stay 128-bit loads from the reflected / wrapped ROW (plane); only the four
+    // (six) horizontal neighbour values are single loads through the boundary rule.  Same operands in
+    // the same Stencil<>::apply positions as the interior path: the same bits.
 #pragma unroll
-    for (int q = 0; q < NV; ++q) {
-      double2 yy = make_double2(0.0, 0.0), AA = yy, BB = yy;
-      if (KIND != K_SELF) yy = ld2(yb + o + q * a.g.fstride);
-      if (KIND == K_RK4F) { AA = ld2(Ab + o + q * a.g.fstride); BB = ld2(Bb + o + q * a.g.fstride); }
-      double r0 = combine<KIND>(a.w_y, a.w_in, a.w_A, a.w_B, a.w_f, yy.x, z0[q], AA.x, BB.x, f0[q]);
-      double r1 = combine<KIND>(a.w_y, a.w_in, a.w_A, a.w_B, a.w_f, yy.y, z1[q], AA.y, BB.y, f1[q]);
-      st2(ob + o + q * a.g.fstride, r0, r1);
+    for (int q = 0; q < NV; ++q) zz[q] = ld2(in + o + q * a.g.fstride);
+    const int xw1 = bidx(x - 1, nx, bc), xe1 = bidx(x + 2, nx, bc);
+    const int rs1 = bidx(j - 1, ny, bc) * pitch, rn1 = bidx(j + 1, ny, bc) * pitch;
+#pragma unroll
+    for (int q = 0; q < ND; ++q) {
+      const double* U = in + q * a.g.fstride + pz;
+      const double2 c = zz[q];
+      const double w1 = U[row + xw1], e1 = U[row + xe1];
+      const double2 s = ld2(U + rs1 + x), n = ld2(U + rn1 + x);
+      if (STENCIL == S_LAP5) {
+        s0[q] = Stencil<S_LAP5>::apply(c.x, w1, c.y, s.x, n.x);
+        s1[q] = Stencil<S_LAP5>::apply(c.y, c.x, e1, s.y, n.y);
+      } else if (STENCIL == S_LAP9X4) {
+        const double w2 = U[row + bidx(x - 2, nx, bc)], e2 = U[row + bidx(x + 3, nx, bc)];
+        const double2 a2 = ld2(U + bidx(j - 2, ny, bc) * pitch + x), b2 = ld2(U + bidx(j + 2, ny, bc) * pitch + x);
+        s0[q] = Stencil<S_LAP9X4>::apply(c.x, w1, c.y, s.x, n.x, w2, e1, a2.x, b2.x);
+        s1[q] = Stencil<S_LAP9X4>::apply(c.y, c.x, e1, s.y, n.y, w1, e2, a2.y, b2.y);
+      } else {
+        const double sw = U[rs1 + xw1], se = U[rs1 + xe1], nw = U[rn1 + xw1], ne = U[rn1 + xe1];
+        s0[q] = Stencil<S_BOX9>::apply(c.x, w1, c.y, s.x, n.x, sw, s.y, nw, n.y);
+        s1[q] = Stencil<S_BOX9>::apply(c.y, c.x, e1, s.y, n.y, s.x, se, n.x, ne);
+      }
+      if (D3) {
+        const double* V = in + q * a.g.fstride + row + x;
+        const int nz = a.g.nz, zs = a.g.zstride;
+        const double2 d1 = ld2(V + (long long)bidx(kz - 1, nz, bc) * zs), u1 = ld2(V + (long long)bidx(kz + 1, nz, bc) * zs);
+        if (STENCIL == S_LAP9X4) {
+          const double2 d2 = ld2(V + (long long)bidx(kz - 2, nz, bc) * zs), u2 = ld2(V + (long long)bidx(kz + 2, nz, bc) * zs);
+          s0[q] += StencilZ<S_LAP9X4>::apply(c.x, d1.x, u1.x, d2.x, u2.x);
+          s1[q] += StencilZ<S_LAP9X4>::apply(c.y, d1.y, u1.y, d2.y, u2.y);
+        } else if (STENCIL == S_LAP5) {
+          s0[q] += StencilZ<S_LAP5>::apply(c.x, d1.x, u1.x);
+          s1[q] += StencilZ<S_LAP5>::apply(c.y, d1.y, u1.y);
+        }
+      }
+    }
+  }
+
+  double z0[NV], z1[NV], f0[NV], f1[NV];
+#pragma unroll
+  for (int q = 0; q < NV; ++q) { z0[q] = zz[q].x; z1[q] = zz[q].y; }
+  MD::reaction(a.p, z0, f0);
+  MD::reaction(a.p, z1, f1);
+#pragma unroll
+  for (int q = 0; q < ND; ++q) {
+    f0[q] = fma(a.lapw[q], s0[q], f0[q]);
+    f1[q] = fma(a.lapw[q], s1[q], f1[q]);
+  }
+  if constexpr (KIND == K_RL || KIND == K_IE) {   // BOCF: u by Euler, the gates with frozen coefficients
+    if constexpr (NV == 4) {
+      double al0[3], be0[3], al1[3], be1[3];
+      MD::gates(a.p, z0[0], al0, be0);
+      MD::gates(a.p, z1[0], al1, be1);
+      st2(ob + o, fma(a.dt, f0[0], z0[0]), fma(a.dt, f1[0], z1[0]));
+#pragma unroll
+      for (int g = 0; g < 3; ++g)
+        st2(ob + o + (g + 1) * a.g.fstride, gate_step<KIND>(a.dt, z0[g + 1], al0[g], be0[g]),
+            gate_step<KIND>(a.dt, z1[g + 1], al1[g], be1[g]));
     }
     return;
   }
-
-  // rim blocks: one cell at a time, boundary rule per neighbour
-  if (j >= ny) return;
-  const int bc = a.g.boundary;
 #pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    const int i = x + h;
-    if (i >= nx) break;
-    const int oc = j * pitch + i;        // inside the plane
-    const off_t o = pz + oc;             // inside the field
-    double z[NV], f[NV];
-#pragma unroll
-    for (int q = 0; q < NV; ++q) z[q] = in[o + q * a.g.fstride];
-    MD::reaction(a.p, z, f);
-#pragma unroll
-    for (int q = 0; q < ND; ++q) {
-      double s = stencil_edge<STENCIL>(in + q * a.g.fstride + pz, i, j, nx, ny, pitch, bc, z[q]);
-      if (D3) s += zarm_edge<STENCIL>(in + q * a.g.fstride, oc, kz, a.g.nz, a.g.zstride, bc, z[q]);
-      f[q] = fma(a.lapw[q], s, f[q]);
-    }
-    finish_cell<MD, KIND>(a, yb, Ab, Bb, ob, o, z, f);
+  for (int q = 0; q < NV; ++q) {
+    double2 yy = make_double2(0.0, 0.0), AA = yy, BB = yy;
+    if (KIND != K_SELF) yy = ld2(yb + o + q * a.g.fstride);
+    if (KIND == K_RK4F) { AA = ld2(Ab + o + q * a.g.fstride); BB = ld2(Bb + o + q * a.g.fstride); }
+    double r0 = combine<KIND>(a.w_y, a.w_in, a.w_A, a.w_B, a.w_f, yy.x, z0[q], AA.x, BB.x, f0[q]);
+    double r1 = combine<KIND>(a.w_y, a.w_in, a.w_A, a.w_B, a.w_f, yy.y, z1[q], AA.y, BB.y, f1[q]);
+    st2(ob + o + q * a.g.fstride, r0, r1);
   }
 }
 

@@ -134,7 +134,7 @@ int cardiac_set_stream(cardiac_ctx*, void* cuda_stream);
  * 2 = 48x40 cells, two CTAs per SM, two-field models only, 3 / 4 / 5 = 64x56 / 64x48 / 56x48 cells, two-field models with RK4); STAGE = kernel implementation (0 = by size, 1 = DIRECT: every thread loads
  * its own operands, 2 = RING: persistent CTAs fed by a TMA shared-memory ring; same results
  * bitwise); PAIR, PERSISTENT: 0.  AUTO: PERSISTENT below ~100x100 cells per member, FUSED for the
- * two-field models, PAIR for the four-field model with RK4 from 4 Mi cells (Heun: 12 Mi), else STAGE. */
+ * two-field models, PAIR for the four-field model with RK4 from 1536^2 cells (Heun: 12 Mi), else STAGE. */
 int cardiac_set_plan(cardiac_ctx*, int plan, int param);
 
 /* The plan that cardiac_step will use (resolved from AUTO). */

@@ -124,8 +124,8 @@ int auto_plan(const Problem& pb) {
   if (resident_preferred(pb)) return CARDIAC_PLAN_PERSISTENT;
   if (rk_like && pb.model != CARDIAC_BOCF) return CARDIAC_PLAN_FUSED;
   // 4-field model: two substeps per launch once the grid gives every SM enough tiles (measured on B200,
-  // RK4 2048^2 +4 %, 4096^2 +13 %, 8192^2 +19 % over STAGE, equal at 1536^2, behind
-  // below; Heun +2 % at 4096^2, behind at 2048^2)
+  // RK4 1536^2 +2 %, 2048^2 +6 %, 4096^2 +15 %, 8192^2 +19 % over STAGE, behind at
+  // 1024^2; Heun +2 % at 4096^2, behind at 2048^2)
   if (pb.model == CARDIAC_BOCF) {
     const long long cells = (long long)pb.nx * pb.ny * pb.batch;
     if ((pb.integrator == I_RK4 && cells >= kPairMinCellsRK4) || (pb.integrator == I_HEUN && cells >= kPairMinCellsHeun))

@@ -81,7 +81,8 @@ CARDIAC_D double2 ld2v(const double* p) {
 // PRE (substep B = K_RK4F, tile cells): also forms the part of the final combination that does not
 // depend on substep B's result, P = w_B Y3 + (w_A Y2 + w_y y) — Y3 is this substep's input — and
 // stores it where substep B will write (which may be where Y2 was read: same thread, same cell).
-template <class MD, int STENCIL, int KIND, bool FULL, bool PRE, bool EARLY = false>
+// BC: the pair lies inside the grid but its stencil may reach across the boundary (stencil_pair_bc).
+template <class MD, int STENCIL, int KIND, bool FULL, bool PRE, bool EARLY = false, bool BC = false>
 CARDIAC_D void pair_from_global(const PairArgs<MD>& a, const double* __restrict__ in,
                                 const double* __restrict__ yb, const double* Ab, double* ob, int row, int x,
                                 double2 (&res)[MD::NV]) {
@@ -100,7 +101,10 @@ CARDIAC_D void pair_from_global(const PairArgs<MD>& a, const double* __restrict_
   for (int q = 0; q < NV; ++q) zz[q] = ld2(in + o + q * a.g.fstride);
   double s0[ND], s1[ND];
 #pragma unroll
-  for (int q = 0; q < ND; ++q) stencil_pair<STENCIL>(in + q * a.g.fstride, row, x, a.g.pitch, zz[q], s0[q], s1[q]);
+  for (int q = 0; q < ND; ++q) {
+    if (BC) stencil_pair_bc<STENCIL>(in + q * a.g.fstride, x, row / a.g.pitch, a.g.nx, a.g.ny, a.g.pitch, a.g.boundary, zz[q], s0[q], s1[q]);
+    else stencil_pair<STENCIL>(in + q * a.g.fstride, row, x, a.g.pitch, zz[q], s0[q], s1[q]);
+  }
   // EARLY (tile cells of interior tiles): every global operand of the row is requested before the
   // reaction starts, so that a warp waits for memory once per row; costs 8 registers per operand
   double2 yy[NV], AA[NV];
@@ -214,6 +218,22 @@ __device__ __noinline__ void pair_phase1_rim(const PairArgs<MD>& a, double* __re
         }
       } else {
         pair_from_global<MD, STENCIL, KA, false, false>(a, in, yb, Ab, ob, j * pitch, x, res);
+      }
+#pragma unroll
+      for (int q = 0; q < ND; ++q) *reinterpret_cast<double2*>(swp + q * WSZ) = res[q];
+    } else if (x >= 0 && x + 1 < nx && j >= 0 && j < ny) {
+      // inside the grid, its stencil across the boundary: still 128-bit loads
+      double2 res[NV];
+      if (body) {
+        pair_from_global<MD, STENCIL, KA, true, PRE, false, true>(a, in, yb, Ab, ob, j * pitch, x, res);
+#pragma unroll
+        for (int q = ND; q < NV; ++q) *reinterpret_cast<double2*>(sgp + (q - ND) * TSZ) = res[q];
+        if (STORE_MID) {
+#pragma unroll
+          for (int q = 0; q < NV; ++q) st2(mid + j * pitch + x + q * a.g.fstride, res[q].x, res[q].y);
+        }
+      } else {
+        pair_from_global<MD, STENCIL, KA, false, false, false, true>(a, in, yb, Ab, ob, j * pitch, x, res);
       }
 #pragma unroll
       for (int q = 0; q < ND; ++q) *reinterpret_cast<double2*>(swp + q * WSZ) = res[q];

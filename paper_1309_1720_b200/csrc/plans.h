@@ -77,7 +77,7 @@ struct PairLaunch {
   double a_wy, a_win, a_wf;
   double w_y, w_in, w_A, w_B, w_f;
 };
-constexpr long long kPairMinCellsRK4 = 4LL << 20, kPairMinCellsHeun = 12LL << 20;  // AUTO, 4-field model
+constexpr long long kPairMinCellsRK4 = 9LL << 18, kPairMinCellsHeun = 12LL << 20;  // AUTO, 4-field model: 1536^2, 3584^2
 cudaError_t launch_pair_fhn(const Problem& pb, const PairLaunch& pl, cudaStream_t stream);
 cudaError_t launch_pair_karma(const Problem& pb, const PairLaunch& pl, cudaStream_t stream);
 cudaError_t launch_pair_bocf(const Problem& pb, const PairLaunch& pl, cudaStream_t stream);

@@ -132,6 +132,33 @@ CARDIAC_D double stencil_edge(const double* __restrict__ U, int i, int j, int nx
   }
 }
 
+// ... of a pair (x, x+1) INSIDE the grid whose stencil may reach across the boundary: the pair's vertical
+// neighbours stay 128-bit loads from the reflected / wrapped ROW; only the four (six) horizontal
+// neighbour values are single loads through the boundary rule.  Same operands in the same
+// Stencil<>::apply positions as stencil_pair: the same bits.  U points at the field (plane), x is even.
+template <int STENCIL>
+CARDIAC_D void stencil_pair_bc(const double* __restrict__ U, int x, int j, int nx, int ny, int pitch, int bc,
+                               double2 c, double& s0, double& s1) {
+  const int row = j * pitch;
+  const int xw1 = bidx(x - 1, nx, bc), xe1 = bidx(x + 2, nx, bc);
+  const int rs1 = bidx(j - 1, ny, bc) * pitch, rn1 = bidx(j + 1, ny, bc) * pitch;
+  const double w1 = U[row + xw1], e1 = U[row + xe1];
+  const double2 s = ld2(U + rs1 + x), n = ld2(U + rn1 + x);
+  if (STENCIL == S_LAP5) {
+    s0 = Stencil<S_LAP5>::apply(c.x, w1, c.y, s.x, n.x);
+    s1 = Stencil<S_LAP5>::apply(c.y, c.x, e1, s.y, n.y);
+  } else if (STENCIL == S_LAP9X4) {
+    const double w2 = U[row + bidx(x - 2, nx, bc)], e2 = U[row + bidx(x + 3, nx, bc)];
+    const double2 a2 = ld2(U + bidx(j - 2, ny, bc) * pitch + x), b2 = ld2(U + bidx(j + 2, ny, bc) * pitch + x);
+    s0 = Stencil<S_LAP9X4>::apply(c.x, w1, c.y, s.x, n.x, w2, e1, a2.x, b2.x);
+    s1 = Stencil<S_LAP9X4>::apply(c.y, c.x, e1, s.y, n.y, w1, e2, a2.y, b2.y);
+  } else {
+    const double sw = U[rs1 + xw1], se = U[rs1 + xe1], nw = U[rn1 + xw1], ne = U[rn1 + xe1];
+    s0 = Stencil<S_BOX9>::apply(c.x, w1, c.y, s.x, n.x, sw, s.y, nw, n.y);
+    s1 = Stencil<S_BOX9>::apply(c.y, c.x, e1, s.y, n.y, s.x, se, n.x, ne);
+  }
+}
+
 // 3-D: what the z axis adds to the integer-weight sum of the 2-D stencil of the same family
 // (7-point = LAP5 + z arm, 13-point = LAP9X4 + z arm; same per-axis weights, DESIGN.md f4)
 template <int STENCIL>

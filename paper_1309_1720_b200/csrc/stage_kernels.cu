@@ -165,33 +165,14 @@ __global__ void __launch_bounds__(TX * TY, 8)
       finish_cell<MD, KIND>(a, yb, Ab, Bb, ob, o, z, f);
       return;
     }
-    // A pair inside the grid whose stencil may reach across the boundary: the pair and its vertical
-    // (and z) neighbours stay 128-bit loads from the reflected / wrapped ROW (plane); only the four
-    // (six) horizontal neighbour values are single loads through the boundary rule.  Same operands in
-    // the same Stencil<>::apply positions as the interior path: the same bits.
+    // A pair inside the grid whose stencil may reach across the boundary keeps its 128-bit loads
+    // (stencil_pair_bc, stage.cuh); in 3-D the z neighbours come from the reflected / wrapped plane.
 #pragma unroll
     for (int q = 0; q < NV; ++q) zz[q] = ld2(in + o + q * a.g.fstride);
-    const int xw1 = bidx(x - 1, nx, bc), xe1 = bidx(x + 2, nx, bc);
-    const int rs1 = bidx(j - 1, ny, bc) * pitch, rn1 = bidx(j + 1, ny, bc) * pitch;
 #pragma unroll
     for (int q = 0; q < ND; ++q) {
-      const double* U = in + q * a.g.fstride + pz;
       const double2 c = zz[q];
-      const double w1 = U[row + xw1], e1 = U[row + xe1];
-      const double2 s = ld2(U + rs1 + x), n = ld2(U + rn1 + x);
-      if (STENCIL == S_LAP5) {
-        s0[q] = Stencil<S_LAP5>::apply(c.x, w1, c.y, s.x, n.x);
-        s1[q] = Stencil<S_LAP5>::apply(c.y, c.x, e1, s.y, n.y);
-      } else if (STENCIL == S_LAP9X4) {
-        const double w2 = U[row + bidx(x - 2, nx, bc)], e2 = U[row + bidx(x + 3, nx, bc)];
-        const double2 a2 = ld2(U + bidx(j - 2, ny, bc) * pitch + x), b2 = ld2(U + bidx(j + 2, ny, bc) * pitch + x);
-        s0[q] = Stencil<S_LAP9X4>::apply(c.x, w1, c.y, s.x, n.x, w2, e1, a2.x, b2.x);
-        s1[q] = Stencil<S_LAP9X4>::apply(c.y, c.x, e1, s.y, n.y, w1, e2, a2.y, b2.y);
-      } else {
-        const double sw = U[rs1 + xw1], se = U[rs1 + xe1], nw = U[rn1 + xw1], ne = U[rn1 + xe1];
-        s0[q] = Stencil<S_BOX9>::apply(c.x, w1, c.y, s.x, n.x, sw, s.y, nw, n.y);
-        s1[q] = Stencil<S_BOX9>::apply(c.y, c.x, e1, s.y, n.y, s.x, se, n.x, ne);
-      }
+      stencil_pair_bc<STENCIL>(in + q * a.g.fstride + pz, x, j, nx, ny, pitch, bc, c, s0[q], s1[q]);
       if (D3) {
         const double* V = in + q * a.g.fstride + row + x;
         const int nz = a.g.nz, zs = a.g.zstride;

@@ -48,8 +48,20 @@ CARDIAC_D unsigned cluster_rank() {
   asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
   return r;
 }
+// Full cluster barrier with release / acquire at cluster scope: orders global AND shared memory (ptxas:
+// MEMBAR.ALL.GPU before the arrive, CCTL.IVALL after the wait).  Used where global memory is involved
+// (after the load, before the exit).
 CARDIAC_D void cluster_sync_all() {
   asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// The barrier between substeps orders SHARED memory only: every thread's stage results are st.shared to
+// its own CTA's buffer, and the readers are ld.shared::cluster of other CTAs, served by the shared
+// memory of the SM that owns the buffer — the only copy there is.  fence.acq_rel.cta (MEMBAR.ALL.CTA)
+// holds the arrive back until this thread's stores have been performed there; the arrive itself is
+// relaxed, which drops the GPU-scope MEMBAR of the release form (measured on B200, 64^2: FHN Euler
+// 0.98 -> 0.83 us per step, BOCF RK4 13.9 -> 11.5 us); the wait keeps its acquire.
+CARDIAC_D void cluster_sync_shared() {
+  asm volatile("fence.acq_rel.cta;\n\tbarrier.cluster.arrive.relaxed.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 // the value at the same shared-memory offset as `p` in CTA `rank` of the cluster
 CARDIAC_D double ld_cluster(const double* p, unsigned rank) {
@@ -196,7 +208,7 @@ struct ResidentEngine {
       double* c = sm + cur * ND * fsz;
       double* n = sm + (cur ^ 1) * ND * fsz;
       stage<S>(a, c, n, st);
-      cluster_sync_all();
+      cluster_sync_shared();
       fill_ghosts(a, n, y0, rows, rank, st);
       cur ^= 1;
       stages_from<S + 1>(a, sm, cur, st, y0, rows, rank);

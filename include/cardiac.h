@@ -70,8 +70,9 @@ enum {
                                   overlapped tiles, one launch                                  */
   CARDIAC_PLAN_PERSISTENT = 3, /* ONE launch for all nsteps: each batch member resident in the shared
                                   memory of a thread-block cluster (<= 8 CTAs), ghost rows exchanged
-                                  through distributed shared memory; grids up to 8 x 4096 cells
-                                  (4-field model: 8 x 2048); Euler, Heun, RK4                   */
+                                  through distributed shared memory; grids up to C x 4096 cells
+                                  (4-field model: C x 2048), C = 16 CTAs for batches of up to 4
+                                  members, else 8; Euler, Heun, RK4                             */
   CARDIAC_PLAN_PAIR       = 4  /* two consecutive substeps per launch: the first on tile + ring into
                                   shared memory, the second from there (RK4: two launches, the fourth
                                   stage value never reaches memory; Heun: one launch; Euler: two time
@@ -133,7 +134,7 @@ int cardiac_set_stream(cardiac_ctx*, void* cuda_stream);
  * launch (0 = default); FUSED + Heun/RK4 = window (0 = by size, 1 = 80x48 cells, one CTA per SM,
  * 2 = 48x40 cells, two CTAs per SM, two-field models only, 3 / 4 / 5 = 64x56 / 64x48 / 56x48 cells, two-field models with RK4); STAGE = kernel implementation (0 = by size, 1 = DIRECT: every thread loads
  * its own operands, 2 = RING: persistent CTAs fed by a TMA shared-memory ring; same results
- * bitwise); PAIR, PERSISTENT: 0.  AUTO: PERSISTENT below ~100x100 cells per member, FUSED for the
+ * bitwise); PAIR, PERSISTENT: 0.  AUTO: PERSISTENT below ~120x120 .. 180x180 cells per member (by model and integrator; batches of up to 4 members, half of that up to 16), FUSED for the
  * two-field models, PAIR for the four-field model with RK4 from 1536^2 cells (Heun: 12 Mi), else STAGE. */
 int cardiac_set_plan(cardiac_ctx*, int plan, int param);
 

@@ -475,7 +475,7 @@ int cardiac_set_plan(cardiac_ctx* c, int plan, int param) {
   } else if (resolved == CARDIAC_PLAN_PERSISTENT) {
     if (!resident_supported(c->pb))
       return fail(c, CARDIAC_ERR_INVALID,
-                  "PERSISTENT needs Euler/Heun/RK4 and a grid that fits one cluster: 8 x 4096 cells (4-field model: 8 x 2048)");
+                  "PERSISTENT needs Euler/Heun/RK4 and a grid that fits one cluster: C x 4096 cells (4-field model: C x 2048), C = 16 CTAs for batches of up to 4 members, else 8");
     if (param != 0) return fail(c, CARDIAC_ERR_INVALID, "plan parameter must be 0");
   } else {
     return fail(c, CARDIAC_ERR_INVALID, "plan not available for this context");

@@ -90,7 +90,8 @@ inline cudaError_t launch_pair(const Problem& pb, const PairLaunch& pl, cudaStre
 // resident_kernels_*.cu: plan PERSISTENT — one thread-block cluster of C <= 8 CTAs per batch member
 // keeps the whole grid in (distributed) shared memory and advances all nsteps in ONE launch, in place
 // (resident.cuh).  C CTAs of 512 threads x KP pairs: at most C x 4096 cells (2-field models) or
-// C x 2048 cells (4-field model); Euler / Heun / RK4.
+// C x 2048 cells (4-field model), C <= 16 for batches of up to 4 members (the non-portable cluster size)
+// and <= 8 beyond; Euler / Heun / RK4.
 struct ResidentLaunch {
   double* state;
   long long nsteps;
@@ -105,12 +106,13 @@ inline ResidentShape resident_shape(const Problem& pb) {
   if (pb.integrator > 2 || pb.nz > 1) return rs;  // Euler, Heun, RK4; 2-D
   const long long npx = (pb.nx + 1) / 2, cap = 512LL * (pb.nv > 2 ? 2 : 4);
   const size_t sp = 2 * (size_t)npx + 4;
-  for (int c = 1; c <= 8; c *= 2) {
+  const int cmax = pb.batch <= 4 ? 16 : 8;   // 16: non-portable size, at most one such cluster per GPC
+  for (int c = 1; c <= cmax; c *= 2) {
     const int slab = (pb.ny + c - 1) / c;
     const size_t smem = 2 * (size_t)pb.nd * sp * ((size_t)slab + 2 * pb.radius) * sizeof(double);
-    // fits, and one pair per thread where the grid is large enough to spread (the substep is
-    // bound by the barrier, not by arithmetic, below that)
-    if (npx * slab <= cap && smem <= 200 * 1024 && (npx * slab <= 512 || c == 8)) {
+    // fits, and one cell per thread where the grid is large enough to spread (a substep costs the
+    // barrier plus the latency of one warp's instruction sequence, resident.cuh CPT)
+    if (npx * slab <= cap && smem <= 200 * 1024 && (c == cmax || (pb.ny + 2 * c - 1) / (2 * c) < 4)) {
       rs.csize = c; rs.slab = slab; rs.smem = smem;
       return rs;
     }
@@ -118,12 +120,21 @@ inline ResidentShape resident_shape(const Problem& pb) {
   return rs;
 }
 inline bool resident_supported(const Problem& pb) { return resident_shape(pb).csize > 0; }
-// AUTO: measured on B200, one cluster-resident launch beats the per-step
-// launches of FUSED / STAGE up to about 100 x 100 cells per member (a substep costs ~1 us of
-// barrier + ghost exchange whatever the size), as long as the batch does not already fill the GPU
+// AUTO: measured on B200: a substep of the cluster-resident launch costs the barrier,
+// the ghost exchange and the latency of one warp's instruction sequence, which grows with the cells a
+// CTA holds; against the per-step launches of FUSED / STAGE it wins up to (batch 1, 16 CTAs) 180^2 for
+// FHN Euler, 120^2 for FHN RK4, 140^2 for Karma RK4, 128^2 for BOCF (one cell per thread) — expressed per
+// CTA so that it carries over to the 8-CTA clusters of larger batches — and only while every cluster is
+// resident at once (a GPC holds one cluster of 16, two of 8, four of 4: 17 members in clusters of 8 run
+// as two waves, 8.0 against 6.0 us per FHN RK4 step at 64^2).
 inline bool resident_preferred(const Problem& pb) {
   const ResidentShape rs = resident_shape(pb);
-  return rs.csize > 0 && (long long)((pb.nx + 1) / 2) * pb.ny <= 5120 && (long long)pb.batch * rs.csize <= 296;
+  if (rs.csize == 0) return false;
+  const int max_clusters = rs.csize == 16 ? 4 : (rs.csize == 8 ? 16 : (rs.csize == 4 ? 32 : 144 / rs.csize));
+  if (pb.batch > max_clusters) return false;
+  const long long cells_per_cta = 2LL * ((pb.nx + 1) / 2) * rs.slab;
+  const long long limit = pb.nv > 2 ? 1024 : (pb.integrator == 0 ? 2048 : (pb.model == 0 ? 900 : 1200));
+  return cells_per_cta <= limit;
 }
 cudaError_t launch_resident_fhn(const Problem& pb, const ResidentLaunch& rl, cudaStream_t stream);
 cudaError_t launch_resident_karma(const Problem& pb, const ResidentLaunch& rl, cudaStream_t stream);

@@ -72,7 +72,12 @@ CARDIAC_D double ld_cluster(const double* p, unsigned rank) {
   return v;
 }
 
-template <class MD, int STENCIL, int INTEG, int KP>
+// CPT = cells per thread and unit: 2 = an x-adjacent pair (128-bit shared-memory accesses); 1 = ONE cell
+// of the pair, the even warps taking the first and the odd warps the second cell of the same 32 pairs
+// (warp-uniform, so each branch keeps only its half of stencil_pair): a substep of a small grid is bound
+// by the latency of one warp's dependent instruction sequence, and half the sequence in twice the warps
+// halves it.  Same per-cell instruction sequence, same bits.
+template <class MD, int STENCIL, int INTEG, int KP, int CPT>
 struct ResidentEngine {
   static constexpr int NV = MD::NV, ND = MD::ND, NG = NV - ND;
   static constexpr int R = stencil_radius(STENCIL);
@@ -95,10 +100,10 @@ struct ResidentEngine {
     unsigned owner;
   };
   struct Patch {
-    double y[RK ? KP : 1][2][NV];
-    double acc[RK ? KP : 1][2][NV];
-    double g[KP][2][NG > 0 ? NG : 1];
-    int off[KP];   // offset of the pair inside a shared field, -1 = no such pair
+    double y[RK ? KP : 1][CPT][NV];
+    double acc[RK ? KP : 1][CPT][NV];
+    double g[KP][CPT][NG > 0 ? NG : 1];
+    int off[KP];   // offset of the pair inside a shared field, -1 = no such pair (CPT = 1: or no such cell)
     Ghost gh[GK];  // dst < 0: none
   };
   CARDIAC_D static Ghost ghost_entry(const ResidentArgs<MD>& a, int e, int y0, int rows, unsigned rank) {
@@ -151,52 +156,87 @@ struct ResidentEngine {
     }
   }
 
-  // Substep S of every owned pair: reads `cur`, writes the diffusing fields of `nxt`.
+  // pair index of unit k of this thread, and (CPT = 1) which cell of the pair the thread owns
+  CARDIAC_D static int unit_pair(int k) {
+    if (CPT == 2) return threadIdx.x + k * NT;
+    return ((threadIdx.x >> 6) << 5) + (threadIdx.x & 31) + k * (NT / 2);
+  }
+  CARDIAC_D static int unit_half() { return (threadIdx.x >> 5) & 1; }
+
+  // Substep S of unit k at shared offset o.  W = 2: both cells of the pair (register slots 0, 1);
+  // W = 0 / 1: that cell only (slot 0) — the other half of stencil_pair is dead code.
+  template <int S, int W>
+  CARDIAC_D static void stage_unit(const ResidentArgs<MD>& a, const double* __restrict__ cur,
+                                   double* __restrict__ nxt, Patch& st, int k, int o) {
+    constexpr bool LAST = (S == NS - 1);
+    const int fsz = a.sp * a.sr;
+    double2 ctr[ND];
+    double s0[ND], s1[ND];
+#pragma unroll
+    for (int q = 0; q < ND; ++q) {
+      ctr[q] = ld2(cur + q * fsz + o);
+      stencil_pair<STENCIL>(cur + q * fsz, o, 0, a.sp, ctr[q], s0[q], s1[q]);
+    }
+    double res[2][NV];
+#pragma unroll
+    for (int h = (W == 2 ? 0 : W); h < (W == 2 ? 2 : W + 1); ++h) {
+      const int sl = W == 2 ? h : 0;   // register slot
+      double z[NV], f[NV];
+#pragma unroll
+      for (int q = 0; q < NV; ++q)
+        z[q] = q < ND ? (h == 0 ? ctr[q < ND ? q : 0].x : ctr[q < ND ? q : 0].y)
+                      : st.g[k][sl][q >= ND ? q - ND : 0];
+      MD::reaction(a.p, z, f);
+#pragma unroll
+      for (int q = 0; q < ND; ++q) f[q] = fma(a.lapw[q], h == 0 ? s0[q] : s1[q], f[q]);
+#pragma unroll
+      for (int q = 0; q < NV; ++q) {
+        double nv;
+        if (!RK) {
+          nv = fma(a.a_dt[0], f[q], z[q]);
+        } else if (LAST) {
+          nv = fma(a.b_dt[S], f[q], S == 0 ? st.y[k][sl][q] : st.acc[k][sl][q]);
+          st.y[k][sl][q] = nv;   // the next time step starts here
+        } else {
+          st.acc[k][sl][q] = fma(a.b_dt[S], f[q], S == 0 ? st.y[k][sl][q] : st.acc[k][sl][q]);
+          nv = fma(a.a_dt[S], f[q], st.y[k][sl][q]);
+        }
+        res[h][q] = nv;
+        if (q >= ND) st.g[k][sl][q >= ND ? q - ND : 0] = nv;
+      }
+    }
+#pragma unroll
+    for (int q = 0; q < ND; ++q) {
+      if (W == 2) st2(nxt + q * fsz + o, res[0][q], res[1][q]);
+      else nxt[q * fsz + o + W] = res[W][q];
+    }
+  }
+
+  // Substep S of every owned unit: reads `cur`, writes the diffusing fields of `nxt`.
   template <int S>
   CARDIAC_D static void stage(const ResidentArgs<MD>& a, const double* __restrict__ cur,
                               double* __restrict__ nxt, Patch& st) {
-    constexpr bool LAST = (S == NS - 1);
-    const int fsz = a.sp * a.sr;
+    if constexpr (CPT == 2) {
 #pragma unroll
-    for (int k = 0; k < KP; ++k) {
-      const int o = st.off[k];
-      if (o < 0) break;
-      double2 ctr[ND];
-      double s0[ND], s1[ND];
-#pragma unroll
-      for (int q = 0; q < ND; ++q) {
-        ctr[q] = ld2(cur + q * fsz + o);
-        stencil_pair<STENCIL>(cur + q * fsz, o, 0, a.sp, ctr[q], s0[q], s1[q]);
+      for (int k = 0; k < KP; ++k) {
+        const int o = st.off[k];
+        if (o < 0) break;
+        stage_unit<S, 2>(a, cur, nxt, st, k, o);
       }
-      double res[2][NV];
+    } else if (unit_half() == 0) {   // warp-uniform
 #pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        double z[NV], f[NV];
-#pragma unroll
-        for (int q = 0; q < NV; ++q)
-          z[q] = q < ND ? (h == 0 ? ctr[q < ND ? q : 0].x : ctr[q < ND ? q : 0].y)
-                        : st.g[k][h][q >= ND ? q - ND : 0];
-        MD::reaction(a.p, z, f);
-#pragma unroll
-        for (int q = 0; q < ND; ++q) f[q] = fma(a.lapw[q], h == 0 ? s0[q] : s1[q], f[q]);
-#pragma unroll
-        for (int q = 0; q < NV; ++q) {
-          double nv;
-          if (!RK) {
-            nv = fma(a.a_dt[0], f[q], z[q]);
-          } else if (LAST) {
-            nv = fma(a.b_dt[S], f[q], S == 0 ? st.y[k][h][q] : st.acc[k][h][q]);
-            st.y[k][h][q] = nv;   // the next time step starts here
-          } else {
-            st.acc[k][h][q] = fma(a.b_dt[S], f[q], S == 0 ? st.y[k][h][q] : st.acc[k][h][q]);
-            nv = fma(a.a_dt[S], f[q], st.y[k][h][q]);
-          }
-          res[h][q] = nv;
-          if (q >= ND) st.g[k][h][q >= ND ? q - ND : 0] = nv;
-        }
+      for (int k = 0; k < KP; ++k) {
+        const int o = st.off[k];
+        if (o < 0) break;
+        stage_unit<S, 0>(a, cur, nxt, st, k, o);
       }
+    } else {
 #pragma unroll
-      for (int q = 0; q < ND; ++q) st2(nxt + q * fsz + o, res[0][q], res[1][q]);
+      for (int k = 0; k < KP; ++k) {
+        const int o = st.off[k];
+        if (o < 0) break;
+        stage_unit<S, 1>(a, cur, nxt, st, k, o);
+      }
     }
   }
 
@@ -225,22 +265,31 @@ struct ResidentEngine {
     const int fsz = a.sp * a.sr, npairs = a.npx * rows;
     Patch st;
     // load: diffusing fields -> shared buffer 0, gating fields and y -> registers
+    const int half = unit_half();
 #pragma unroll
     for (int k = 0; k < KP; ++k) {
-      const int p = threadIdx.x + k * NT;
+      const int p = unit_pair(k);
       st.off[k] = -1;
       if (p >= npairs) continue;
       const int py = p / a.npx, px = p - py * a.npx, gx = 2 * px;
+      if (CPT == 1 && gx + half >= nx) continue;   // the second cell of the last pair of an odd row
       st.off[k] = (py + R) * a.sp + GX + gx;
 #pragma unroll
       for (int q = 0; q < NV; ++q) {
         const double* f = in + q * a.g.fstride + (long long)(y0 + py) * pitch + gx;
-        double2 v;
-        v.x = f[0];
-        v.y = gx + 1 < nx ? f[1] : 0.0;
-        if (q < ND) st2(sm + q * fsz + st.off[k], v.x, v.y);
-        else { st.g[k][0][q >= ND ? q - ND : 0] = v.x; st.g[k][1][q >= ND ? q - ND : 0] = v.y; }
-        if (RK) { st.y[k][0][q] = v.x; st.y[k][1][q] = v.y; }
+        if constexpr (CPT == 2) {
+          double2 v;
+          v.x = f[0];
+          v.y = gx + 1 < nx ? f[1] : 0.0;
+          if (q < ND) st2(sm + q * fsz + st.off[k], v.x, v.y);
+          else { st.g[k][0][q >= ND ? q - ND : 0] = v.x; st.g[k][1][q >= ND ? q - ND : 0] = v.y; }
+          if (RK) { st.y[k][0][q] = v.x; st.y[k][1][q] = v.y; }
+        } else {
+          const double v = f[half];
+          if (q < ND) sm[q * fsz + st.off[k] + half] = v;
+          else st.g[k][0][q >= ND ? q - ND : 0] = v;
+          if (RK) st.y[k][0][q] = v;
+        }
       }
     }
     {
@@ -260,29 +309,33 @@ struct ResidentEngine {
     const double* c = sm + cur * ND * fsz;
 #pragma unroll
     for (int k = 0; k < KP; ++k) {
-      const int p = threadIdx.x + k * NT;
-      if (p >= npairs) break;
+      const int p = unit_pair(k);
+      if (st.off[k] < 0) break;
       const int py = p / a.npx, px = p - py * a.npx, gx = 2 * px;
 #pragma unroll
       for (int q = 0; q < NV; ++q) {
         double* f = out + q * a.g.fstride + (long long)(y0 + py) * pitch + gx;
-        double2 v;
-        if (q < ND) v = ld2(c + q * fsz + st.off[k]);
-        else v = make_double2(st.g[k][0][q >= ND ? q - ND : 0], st.g[k][1][q >= ND ? q - ND : 0]);
-        f[0] = v.x;
-        if (gx + 1 < nx) f[1] = v.y;
+        if constexpr (CPT == 2) {
+          double2 v;
+          if (q < ND) v = ld2(c + q * fsz + st.off[k]);
+          else v = make_double2(st.g[k][0][q >= ND ? q - ND : 0], st.g[k][1][q >= ND ? q - ND : 0]);
+          f[0] = v.x;
+          if (gx + 1 < nx) f[1] = v.y;
+        } else {
+          f[half] = q < ND ? c[q * fsz + st.off[k] + half] : st.g[k][0][q >= ND ? q - ND : 0];
+        }
       }
     }
     cluster_sync_all();   // nobody leaves while a neighbour may still read its shared memory
   }
 };
 
-template <class MD, int STENCIL, int INTEG, int KP>
+template <class MD, int STENCIL, int INTEG, int KP, int CPT>
 __global__ void __launch_bounds__(kResidentThreads, 1)
     resident_kernel(const __grid_constant__ ResidentArgs<MD> a) {
   extern __shared__ double2 smem_resident[];
   const long long base = (long long)(blockIdx.x / a.csize) * a.g.bstride;
-  ResidentEngine<MD, STENCIL, INTEG, KP>::run(a, a.in + base, a.out + base,
+  ResidentEngine<MD, STENCIL, INTEG, KP, CPT>::run(a, a.in + base, a.out + base,
                                               reinterpret_cast<double*>(smem_resident));
 }
 

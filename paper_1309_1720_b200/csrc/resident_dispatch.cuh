@@ -13,11 +13,11 @@ struct ResidentPairs {
   static constexpr int KP = MD::NV > 2 ? 2 : 4;
 };
 
-template <class MD, int STENCIL, int INTEG>
+template <class MD, int STENCIL, int INTEG, int CPT>
 cudaError_t resident_run(const Problem& pb, const ResidentLaunch& rl, cudaStream_t stream) {
   constexpr int KP = ResidentPairs<MD>::KP;
   constexpr int R = stencil_radius(STENCIL);
-  auto kern = resident_kernel<MD, STENCIL, INTEG, KP>;
+  auto kern = resident_kernel<MD, STENCIL, INTEG, KP, CPT>;
   ResidentArgs<MD> a;
   a.in = rl.state; a.out = rl.state;
   a.g.nx = pb.nx; a.g.ny = pb.ny; a.g.pitch = pb.pitch; a.g.boundary = pb.boundary;
@@ -44,7 +44,13 @@ cudaError_t resident_run(const Problem& pb, const ResidentLaunch& rl, cudaStream
   MD::derive(pb.params, a.p);
   for (int q = 0; q < MD::ND; ++q) a.lapw[q] = a.p.D[q] * stencil_norm(STENCIL) / (pb.dx * pb.dx);
   const size_t smem = rs.smem;
-  if ((long long)a.npx * rs.slab > (long long)kResidentThreads * KP) return cudaErrorInvalidValue;
+  if ((long long)a.npx * rs.slab * (3 - CPT) > (long long)kResidentThreads * KP) return cudaErrorInvalidValue;
+  static bool nonportable = false;
+  if (rs.csize > 8 && !nonportable) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    if (e != cudaSuccess) return e;
+    nonportable = true;
+  }
   static size_t configured = 0;  // per instantiation
   if (smem > configured) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -68,10 +74,17 @@ cudaError_t resident_run(const Problem& pb, const ResidentLaunch& rl, cudaStream
 
 template <class MD, int STENCIL>
 cudaError_t resident_by_integrator(const Problem& pb, const ResidentLaunch& rl, cudaStream_t s) {
+  // one cell per thread and unit where the slab leaves the threads the room (resident.cuh, CPT)
+  const ResidentShape rs = resident_shape(pb);
+  // FHN only while every thread has at most one unit: a thread's units run one after the other, and two
+  // light cells cost more than one pair (Euler 96^2: 1.24 us per step as cells, 0.95 as pairs); Karma and
+  // BOCF wherever the cells fit (Karma RK4 96^2: 5.9 against 6.9 us, BOCF RK4 80^2: 8.5 against 10.8 us)
+  const long long ncell = 2LL * ((pb.nx + 1) / 2) * rs.slab;
+  const bool cells = ncell <= (long long)kResidentThreads * (MD::NV > 2 || pb.model != 0 ? ResidentPairs<MD>::KP : 1);
   switch (pb.integrator) {
-    case I_EULER: return resident_run<MD, STENCIL, I_EULER>(pb, rl, s);
-    case I_HEUN: return resident_run<MD, STENCIL, I_HEUN>(pb, rl, s);
-    case I_RK4: return resident_run<MD, STENCIL, I_RK4>(pb, rl, s);
+    case I_EULER: return cells ? resident_run<MD, STENCIL, I_EULER, 1>(pb, rl, s) : resident_run<MD, STENCIL, I_EULER, 2>(pb, rl, s);
+    case I_HEUN: return cells ? resident_run<MD, STENCIL, I_HEUN, 1>(pb, rl, s) : resident_run<MD, STENCIL, I_HEUN, 2>(pb, rl, s);
+    case I_RK4: return cells ? resident_run<MD, STENCIL, I_RK4, 1>(pb, rl, s) : resident_run<MD, STENCIL, I_RK4, 2>(pb, rl, s);
   }
   return cudaErrorInvalidValue;
 }

@@ -127,11 +127,15 @@ def test_parity_persistent_plan(C, model, stencil, integ):
 @pytest.mark.parametrize("model,stencil,nx,ny,bc", [(FHN, LAP9X4, 5, 5, 0), (KARMA, BOX9, 3, 3, 0), (FHN, LAP9X4, 64, 64, 1),
                                                     (KARMA, LAP5, 33, 4, 1), (BOCF, LAP9X4, 64, 32, 0), (BOCF, BOX9, 37, 50, 1),
                                                     (FHN, LAP9X4, 1000, 9, 0), (KARMA, BOX9, 176, 176, 1),
-                                                    (BOCF, LAP9X4, 128, 125, 0), (FHN, BOX9, 90, 61, 0)])
+                                                    (BOCF, LAP9X4, 128, 125, 0), (FHN, BOX9, 90, 61, 0),
+                                                    (FHN, LAP9X4, 250, 250, 0), (BOCF, BOX9, 180, 176, 1),
+                                                    (KARMA, LAP9X4, 2000, 9, 0), (FHN, LAP5, 131, 97, 1)])
 def test_parity_persistent_edges(C, model, stencil, nx, ny, bc):
     """Minimum sizes (one CTA), the periodic boundary across the cluster (the first slab reads the
     last one), slabs of r rows with empty trailing CTAs (1000 x 9 over 8 CTAs), the capacity limits
-    (8 x 4096 / 8 x 2048 cells) and a ragged last slab (61 rows over 8 CTAs)."""
+    (8 x 4096 / 8 x 2048 cells) and a ragged last slab (61 rows over 8 CTAs); clusters of 16 CTAs (batches
+    of up to 4 members) at their capacity (250 x 250: 16 slabs of 16 rows x 125 pairs; 180 x 176 for the
+    4-field model), slabs of r rows (2000 x 9 over 8 CTAs) and odd widths in one-cell-per-thread mode."""
     cfg, Z = make(model, nx, ny, stencil, RK4, boundary=bc)
     got = gpu_run(C, cfg, Z, 30, plan=PERSISTENT)
     ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 30)
@@ -139,7 +143,7 @@ def test_parity_persistent_edges(C, model, stencil, nx, ny, bc):
 
 
 def test_persistent_plan_limits_and_auto(C):
-    cfg, _ = make(FHN, 200, 200, LAP5, RK4)                    # 40000 cells: more than 8 x 4096
+    cfg, _ = make(FHN, 300, 300, LAP5, RK4)                    # 90000 cells: more than 16 x 4096
     with C.Context.from_config(cfg) as ctx:
         assert ctx.plan == FUSED
         with pytest.raises(C.CardiacError):
@@ -154,6 +158,19 @@ def test_persistent_plan_limits_and_auto(C):
         assert ctx.plan == 1
         with pytest.raises(C.CardiacError):
             C.cardiac_set_plan(ctx.ctx, PERSISTENT, 0)
+    # clusters of 16 CTAs for up to 4 members, of 8 beyond: the same bits, member by member
+    cfg6, Z6 = make(KARMA, 64, 64, LAP9X4, RK4, batch=6)
+    got6 = gpu_run(C, cfg6, Z6, 20, plan=PERSISTENT)
+    cfg1, _ = make(KARMA, 64, 64, LAP9X4, RK4)
+    for b in (0, 5):
+        assert np.array_equal(got6[b:b + 1], gpu_run(C, cfg1, Z6[b:b + 1], 20, plan=PERSISTENT))
+    # AUTO: every cluster must be resident at once (17 members in clusters of 8 are two waves)
+    cfg, _ = make(FHN, 64, 64, LAP9X4, RK4, batch=17)
+    with C.Context.from_config(cfg) as ctx:
+        assert ctx.plan == FUSED
+    cfg, _ = make(KARMA, 128, 128, LAP5, RK4)
+    with C.Context.from_config(cfg) as ctx:
+        assert ctx.plan == PERSISTENT
 
 
 @pytest.mark.parametrize("model,stencil,integ", [(FHN, LAP9X4, RK4), (KARMA, LAP5, RK4), (BOCF, LAP9X4, RK4),

@@ -227,14 +227,14 @@ struct ResidentEngine {
 #pragma unroll
       for (int k = 0; k < KP; ++k) {
         const int o = st.off[k];
-        if (o < 0) break;
+        if (o < 0) continue;   // (an odd row has no second cell in its last pair; a later unit may exist)
         stage_unit<S, 0>(a, cur, nxt, st, k, o);
       }
     } else {
 #pragma unroll
       for (int k = 0; k < KP; ++k) {
         const int o = st.off[k];
-        if (o < 0) break;
+        if (o < 0) continue;
         stage_unit<S, 1>(a, cur, nxt, st, k, o);
       }
     }
@@ -310,7 +310,7 @@ struct ResidentEngine {
 #pragma unroll
     for (int k = 0; k < KP; ++k) {
       const int p = unit_pair(k);
-      if (st.off[k] < 0) break;
+      if (st.off[k] < 0) continue;
       const int py = p / a.npx, px = p - py * a.npx, gx = 2 * px;
 #pragma unroll
       for (int q = 0; q < NV; ++q) {

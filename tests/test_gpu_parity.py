@@ -129,13 +129,14 @@ def test_parity_persistent_plan(C, model, stencil, integ):
                                                     (FHN, LAP9X4, 1000, 9, 0), (KARMA, BOX9, 176, 176, 1),
                                                     (BOCF, LAP9X4, 128, 125, 0), (FHN, BOX9, 90, 61, 0),
                                                     (FHN, LAP9X4, 250, 250, 0), (BOCF, BOX9, 180, 176, 1),
-                                                    (KARMA, LAP9X4, 2000, 9, 0), (FHN, LAP5, 131, 97, 1)])
+                                                    (KARMA, LAP9X4, 2000, 9, 0), (FHN, LAP5, 131, 97, 1),
+                                                    (KARMA, LAP5, 131, 97, 0), (BOCF, LAP9X4, 75, 100, 0)])
 def test_parity_persistent_edges(C, model, stencil, nx, ny, bc):
     """Minimum sizes (one CTA), the periodic boundary across the cluster (the first slab reads the
     last one), slabs of r rows with empty trailing CTAs (1000 x 9 over 8 CTAs), the capacity limits
     (8 x 4096 / 8 x 2048 cells) and a ragged last slab (61 rows over 8 CTAs); clusters of 16 CTAs (batches
     of up to 4 members) at their capacity (250 x 250: 16 slabs of 16 rows x 125 pairs; 180 x 176 for the
-    4-field model), slabs of r rows (2000 x 9 over 8 CTAs) and odd widths in one-cell-per-thread mode."""
+    4-field model), slabs of r rows (2000 x 9 over 8 CTAs) and odd widths in one-cell-per-thread mode with one and with several cells per thread."""
     cfg, Z = make(model, nx, ny, stencil, RK4, boundary=bc)
     got = gpu_run(C, cfg, Z, 30, plan=PERSISTENT)
     ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 30)

@@ -87,7 +87,7 @@ inline cudaError_t launch_pair(const Problem& pb, const PairLaunch& pl, cudaStre
                                         : launch_pair_bocf(pb, pl, stream));
 }
 
-// resident_kernels_*.cu: plan PERSISTENT — one thread-block cluster of C <= 8 CTAs per batch member
+// resident_kernels_*.cu: plan PERSISTENT — one thread-block cluster of C <= 16 CTAs per batch member
 // keeps the whole grid in (distributed) shared memory and advances all nsteps in ONE launch, in place
 // (resident.cuh).  C CTAs of 512 threads x KP pairs: at most C x 4096 cells (2-field models) or
 // C x 2048 cells (4-field model), C <= 16 for batches of up to 4 members (the non-portable cluster size)

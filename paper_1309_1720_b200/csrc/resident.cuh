@@ -3,7 +3,7 @@
 //
 // The paper's small-grid regime (N < N0 ~ 362, Fig. 5 :166) is bound by the cost of
 // launching (n_d + 2) n_s kernels per time step, not by arithmetic.  Here a batch member is owned
-// by one cluster of C <= 8 CTAs for the whole run; CTA `rank` holds the slab of rows
+// by one cluster of C <= 16 CTAs (8 for batches of more than 4 members) for the whole run; CTA `rank` holds the slab of rows
 // [rank h, rank h + h).  The stage values of the diffusing fields live in two shared-memory buffers
 // framed by a ghost ring of r cells, each thread owns up to KP fixed x-adjacent pairs of cells and
 // keeps their step-start value y, the running RK sum and the gating variables in registers.
@@ -26,7 +26,7 @@
 namespace cardiac {
 
 constexpr int kResidentThreads = 512;
-constexpr int kResidentMaxCluster = 8;   // portable cluster size
+constexpr int kResidentMaxCluster = 16;  // non-portable cluster size (batches of up to 4 members), else 8
 
 template <class MD>
 struct ResidentArgs {

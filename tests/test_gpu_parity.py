@@ -143,6 +143,33 @@ def test_parity_persistent_edges(C, model, stencil, nx, ny, bc):
     assert maxabs(got, ref) <= TOL_100
 
 
+@pytest.mark.parametrize("model,stencil,integ,n,batch,nsteps", [(FHN, LAP5, EULER, 64, 1, 6000), (KARMA, LAP9X4, RK4, 96, 4, 1500),
+                                                                (BOCF, LAP9X4, RK4, 128, 4, 800), (FHN, BOX9, HEUN, 100, 16, 1500)])
+def test_persistent_barrier_stress(C, model, stencil, integ, n, batch, nsteps):
+    """The barrier between substeps orders shared memory only (fence.acq_rel.cta + relaxed cluster
+    arrive + acquire wait, resident.cuh) and compute-sanitizer's racecheck is not available on the
+    GPU pool: a ghost row read before its owner's store had landed, or a buffer overwritten while a
+    neighbour still reads it, would make a long run depend on timing.  Thousands of substeps in one
+    launch (clusters of 16 and of 8, every cluster co-resident), repeated while another stream keeps
+    the other SMs and the L2 busy, and split into launches of other lengths: the same bits every
+    time, and the state still that of the stage-synchronous plan (a stale value is an O(1) error in
+    a cell, far above the roundoff between the two plans)."""
+    import torch
+    cfg, Z = make(model, n, n, stencil, integ, batch=batch)
+    ref = gpu_run(C, cfg, Z, nsteps, plan=PERSISTENT)
+    assert np.isfinite(ref).all() and maxabs(ref, Z) > 1e-6
+    side = torch.cuda.Stream()
+    noise = torch.empty(64 << 20, dtype=torch.float32, device="cuda")
+    for rep in range(4):
+        with torch.cuda.stream(side):
+            for _ in range(20):
+                noise.normal_()
+        assert np.array_equal(ref, gpu_run(C, cfg, Z, nsteps, plan=PERSISTENT))
+    side.synchronize()
+    assert np.array_equal(ref, gpu_run(C, cfg, Z, nsteps, plan=PERSISTENT, chunks=[1, nsteps // 2, nsteps - nsteps // 2 - 1]))
+    assert maxabs(ref, gpu_run(C, cfg, Z, nsteps, plan=STAGE)) <= 1e-8
+
+
 def test_persistent_plan_limits_and_auto(C):
     cfg, _ = make(FHN, 300, 300, LAP5, RK4)                    # 90000 cells: more than 16 x 4096
     with C.Context.from_config(cfg) as ctx:

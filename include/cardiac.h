@@ -182,24 +182,6 @@ int cardiac_get_jvp(cardiac_ctx*, double eps, double* dst, int dst_on_device);
 int cardiac_get_rows(cardiac_ctx*, int j0, int nrows, double* dst, int dst_on_device);
 int cardiac_set_rows(cardiac_ctx*, int j0, int nrows, const double* src, int src_on_device);
 
-/* Diagnostic (not on the hot path): evaluate device-side building blocks on n sample points held
- * in device memory, enqueued on the context stream.
- *   CARDIAC_PROBE_EXP      out[i] = the library's exp(in[i])            (used inside tanh)
- *   CARDIAC_PROBE_RCP      out[i] = the library's 1/in[i], in[i] > 0    (divisions)
- *   CARDIAC_PROBE_HK       out[i] = H_k(in[i]), k of the context's model
- *   CARDIAC_PROBE_REACTION in = [n][n_v] states, out = [n][n_v] reaction terms N[z] of the
- *                          context's model, variant and parameters */
-enum { CARDIAC_PROBE_EXP = 0, CARDIAC_PROBE_RCP = 1, CARDIAC_PROBE_HK = 2, CARDIAC_PROBE_REACTION = 3 };
-int cardiac_probe(cardiac_ctx*, int what, const double* in_dev, double* out_dev, long long n);
-
-/* Total number of kernels this context has launched (graph nodes counted per replay). */
-long long cardiac_launch_count(const cardiac_ctx*);
-
-/* Run `nsteps` steps `reps` times back to back on the context stream and return, via CUDA events
- * recorded on that stream, the device time in milliseconds of the whole run in *ms_total
- * (synchronises the stream).  Used by bench.py for the live per-launch timing of the roofline. */
-int cardiac_time_steps(cardiac_ctx*, long long nsteps, int reps, float* ms_total);
-
 /* Text of the last error on this context; ctx == NULL: the calling thread's last create() error.
  * Never NULL; empty string when there was none. */
 const char* cardiac_last_error(const cardiac_ctx*);

@@ -405,7 +405,8 @@ static void step_once(const problem* q, double* Z, double* w) {
      *   Rush-Larsen:    x+ = x e^{alpha dt} + (beta/alpha)(e^{alpha dt} - 1)   (exponential time differencing)
      *   implicit Euler: x+ = (x + dt beta) / (1 - dt alpha). */
     rhs(q, Z, K1, lapbuf); /* only the u component is used */
-    for (size_t c = 0; c < n; ++c) {
+    OMP_FOR
+    for (long c = 0; c < (long)n; ++c) {
       double alpha[3], beta[3];
       double u = Z[c];
       bocf_gates(q->p, u, q->variant, alpha, beta);

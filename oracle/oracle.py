@@ -9,6 +9,9 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "cardiac_oracle.c")
 _LIBS = {False: os.path.join(_HERE, "liboracle.so"), True: os.path.join(_HERE, "liboracle_omp.so")}
+# the same source for TIMING only (bench.py's cpu_baseline / --impl reference): -O3 -march=native, which
+# lets gcc contract and vectorise; never used for parity (SURVEY.md 8(d) "Oracle timing")
+_TIMING_LIBS = {False: os.path.join(_HERE, "liboracle_fast.so"), True: os.path.join(_HERE, "liboracle_fast_omp.so")}
 _loaded: dict = {}
 
 _dp = ctypes.POINTER(ctypes.c_double)
@@ -26,10 +29,45 @@ def build(force: bool = False) -> None:
         subprocess.run(cmd, check=True)
 
 
-def lib(omp: bool = False) -> ctypes.CDLL:
-    if omp not in _loaded:
-        build()
-        L = ctypes.CDLL(_LIBS[omp])
+def build_timing() -> None:
+    """The timing build, compiled ON THE MACHINE THAT RUNS IT (-march=native): always rebuilt when the
+    marker of this host is missing, so a library built on another CPU model never travels."""
+    marker = os.path.join(_HERE, ".timing_host")
+    host = _cpu_model()
+    fresh = os.path.exists(marker) and open(marker).read() == host
+    for omp, path in _TIMING_LIBS.items():
+        if fresh and os.path.exists(path) and os.path.getmtime(path) >= os.path.getmtime(_SRC):
+            continue
+        cmd = ["gcc", "-O3", "-march=native", "-shared", "-fPIC", "-o", path, _SRC, "-lm"]
+        if omp:
+            cmd.insert(1, "-fopenmp")
+        subprocess.run(cmd, check=True)
+    with open(marker, "w") as fh:
+        fh.write(host)
+
+
+def _cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def cpu_model() -> str:
+    return _cpu_model()
+
+
+def lib(omp: bool = False, timing: bool = False) -> ctypes.CDLL:
+    key = (omp, timing)
+    if key not in _loaded:
+        if timing:
+            build_timing()
+        else:
+            build()
+        L = ctypes.CDLL((_TIMING_LIBS if timing else _LIBS)[omp])
         L.oracle_num_fields.argtypes = [ctypes.c_int]
         L.oracle_num_params.argtypes = [ctypes.c_int]
         L.oracle_default_params.argtypes = [ctypes.c_int, _dp]
@@ -49,8 +87,8 @@ def lib(omp: bool = False) -> ctypes.CDLL:
                                     ctypes.c_double, ctypes.c_int, ctypes.c_int, _dp, _dp,
                                     ctypes.c_longlong]
         L.oracle_jvp.argtypes = [_dp, ctypes.c_int, ctypes.c_size_t, ctypes.c_double, _dp]
-        _loaded[omp] = L
-    return _loaded[omp]
+        _loaded[key] = L
+    return _loaded[key]
 
 
 def threads(omp: bool) -> int:
@@ -153,8 +191,9 @@ def rhs(model: int, Z, dx: float, scheme: int, params=None) -> np.ndarray:
 
 
 def step(model: int, Z, dx: float, dt: float, scheme: int, nsteps: int, params=None,
-         omp: bool = False) -> np.ndarray:
-    """Advance Z ([batch][n_v][ny][nx] or [n_v][ny][nx]) by nsteps; returns a new array."""
+         omp: bool = False, timing: bool = False) -> np.ndarray:
+    """Advance Z ([batch][n_v][ny][nx] or [n_v][ny][nx]) by nsteps; returns a new array.
+    timing=True runs the -O3 -march=native build (bench.py only; never for parity)."""
     Z = np.array(Z, dtype=np.float64, order="C", copy=True)
     shape = Z.shape
     if Z.ndim == 3:
@@ -163,7 +202,7 @@ def step(model: int, Z, dx: float, dt: float, scheme: int, nsteps: int, params=N
     if nv != num_fields(model):
         raise ValueError("wrong number of fields")
     p = None if params is None else _c(params)
-    rc = lib(omp).oracle_step(model, nx, ny, float(dx), float(dt), scheme, batch,
+    rc = lib(omp, timing).oracle_step(model, nx, ny, float(dx), float(dt), scheme, batch,
                               None if p is None else _ptr(p), _ptr(Z), int(nsteps))
     if rc:
         raise ValueError(f"oracle_step failed ({rc})")

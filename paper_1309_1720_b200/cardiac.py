@@ -1,4 +1,5 @@
-"""ctypes binding of libcardiac.so — same names as include/cardiac.h, argument marshalling only.
+"""ctypes binding of libcardiac.so — same names as include/cardiac.h (and the diagnostics of
+include/cardiac_diag.h), argument marshalling only.
 
 Every step of the hot path runs in the library's CUDA kernels; there is no CPU fallback here.
 Importing this module fails loudly if the library has not been built
@@ -31,12 +32,13 @@ CARDIAC_OK, CARDIAC_ERR_INVALID, CARDIAC_ERR_CUDA, CARDIAC_ERR_NOSTATE, CARDIAC_
 
 EXPORTS = [
     "cardiac_num_fields", "cardiac_num_params", "cardiac_default_params", "cardiac_create",
-    "cardiac_set_params", "cardiac_get_params", "cardiac_set_stream", "cardiac_set_plan",
+    "cardiac_create3d",    "cardiac_set_params", "cardiac_get_params", "cardiac_set_stream", "cardiac_set_plan",
     "cardiac_get_plan", "cardiac_workspace_bytes", "cardiac_bind_workspace", "cardiac_set_state",
     "cardiac_step", "cardiac_get_state", "cardiac_get_jvp", "cardiac_get_rows", "cardiac_set_rows",
-    "cardiac_probe", "cardiac_launch_count",
-    "cardiac_time_steps", "cardiac_last_error", "cardiac_destroy",
+    "cardiac_last_error", "cardiac_destroy",
 ]
+# include/cardiac_diag.h: diagnostics for tests and bench.py, not part of the product boundary
+DIAG_EXPORTS = ["cardiac_probe", "cardiac_launch_count", "cardiac_time_steps", "cardiac_measure_fp64_peak"]
 
 
 class CardiacError(RuntimeError):
@@ -73,6 +75,7 @@ _sig = {
     "cardiac_probe": (_i, [_vp, _i, _vp, _vp, _ll]),
     "cardiac_launch_count": (_ll, [_vp]),
     "cardiac_time_steps": (_i, [_vp, _ll, _i, ctypes.POINTER(ctypes.c_float)]),
+    "cardiac_measure_fp64_peak": (_i, [_vp, _i, _i, _dp]),
     "cardiac_last_error": (ctypes.c_char_p, [_vp]),
     "cardiac_destroy": (None, [_vp]),
 }
@@ -210,6 +213,13 @@ def cardiac_time_steps(ctx, nsteps: int, reps: int = 1) -> float:
     ms = ctypes.c_float(0.0)
     _check(ctx, _lib.cardiac_time_steps(ctx, nsteps, reps, ctypes.byref(ms)))
     return float(ms.value)
+
+
+def cardiac_measure_fp64_peak(ctx, iters: int = 2000, reps: int = 5) -> float:
+    """Thread-level DFMA instructions per second of the context's device (include/cardiac_diag.h)."""
+    v = ctypes.c_double(0.0)
+    _check(ctx, _lib.cardiac_measure_fp64_peak(ctx, iters, reps, ctypes.byref(v)))
+    return float(v.value)
 
 
 def cardiac_last_error(ctx=None) -> str:

@@ -10,6 +10,7 @@
 #include <string>
 
 #include "../../include/cardiac.h"
+#include "../../include/cardiac_diag.h"
 #include "plans.h"
 #include "stage.cuh"
 
@@ -301,6 +302,11 @@ int ensure_workspace(cardiac_ctx* c) {
   carve(c);
   return CARDIAC_OK;
 }
+
+// Between two cardiac_step calls only buf[cur] holds data; every other stage buffer is free.  Host-side
+// get_jvp / get_rows / set_rows stage their dense payload there (never larger than a pitched state
+// buffer), so the exchange path allocates nothing and implies no device-wide synchronisation.
+double* scratch_buffer(const cardiac_ctx* c) { return c->buf[(c->cur + 1) % c->nbuf]; }
 
 struct DeviceGuard {
   int prev = -1;
@@ -597,13 +603,11 @@ int cardiac_get_jvp(cardiac_ctx* c, double eps, double* dst, int dst_on_device) 
     c->launches++;
     return CARDIAC_OK;
   }
-  size_t bytes = (size_t)pb.nx * pb.ny * pb.nz * pb.nv * (pb.batch - 1) * sizeof(double);
-  double* tmp = nullptr;
-  CK(cudaMalloc(&tmp, bytes));
+  const size_t bytes = (size_t)pb.nx * pb.ny * pb.nz * pb.nv * (pb.batch - 1) * sizeof(double);
+  double* tmp = scratch_buffer(c);
   cudaError_t e = launch_jvp(pb, c->buf[c->cur], eps, tmp, c->stream);
   if (e == cudaSuccess) e = cudaMemcpyAsync(dst, tmp, bytes, cudaMemcpyDeviceToHost, c->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-  cudaFree(tmp);
   if (e != cudaSuccess) return fail_cuda(c, e, "jvp");
   c->launches++;
   return CARDIAC_OK;
@@ -626,14 +630,12 @@ int rows_copy(cardiac_ctx* c, int j0, int nrows, double* buf, int on_device, boo
     return CARDIAC_OK;
   }
   const size_t bytes = (size_t)pb.batch * pb.nv * nrows * pb.nx * sizeof(double);
-  double* tmp = nullptr;
-  CK(cudaMalloc(&tmp, bytes));
+  double* tmp = scratch_buffer(c);
   cudaError_t e = cudaSuccess;
   if (!pack) e = cudaMemcpyAsync(tmp, buf, bytes, cudaMemcpyHostToDevice, c->stream);
   if (e == cudaSuccess) e = launch_rows(pb, c->buf[c->cur], j0, nrows, tmp, pack, c->stream);
   if (e == cudaSuccess && pack) e = cudaMemcpyAsync(buf, tmp, bytes, cudaMemcpyDeviceToHost, c->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-  cudaFree(tmp);
   if (e != cudaSuccess) return fail_cuda(c, e, "rows copy");
   c->launches++;
   return CARDIAC_OK;
@@ -679,6 +681,38 @@ int cardiac_time_steps(cardiac_ctx* c, long long nsteps, int reps, float* ms_tot
   cudaEventDestroy(e1);
   if (rc) return rc;
   if (e != cudaSuccess) return fail_cuda(c, e, "timing");
+  return CARDIAC_OK;
+}
+
+int cardiac_measure_fp64_peak(cardiac_ctx* c, int iters, int reps, double* dfma_per_s) {
+  if (!c) return CARDIAC_ERR_INVALID;
+  if (!dfma_per_s || iters < 1 || reps < 1) return fail(c, CARDIAC_ERR_INVALID, "bad arguments");
+  DeviceGuard guard(c->device);
+  int sms = 0;
+  CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device));
+  const int blocks = sms * 4;   // 4 x 256 threads = 32 warps per SM, all resident (launch bounds)
+  double* sink = nullptr;
+  CK(cudaMalloc(&sink, (size_t)blocks * kDfmaThreads * sizeof(double)));
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  cudaError_t e = cudaEventCreate(&e0);
+  if (e == cudaSuccess) e = cudaEventCreate(&e1);
+  float best = 0.f;
+  for (int r = 0; r <= reps && e == cudaSuccess; ++r) {   // r = 0: warm-up
+    e = cudaEventRecord(e0, c->stream);
+    if (e == cudaSuccess) e = launch_dfma_peak(sink, blocks, iters, c->stream);
+    if (e == cudaSuccess) e = cudaEventRecord(e1, c->stream);
+    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    if (r > 0 && (best == 0.f || ms < best)) best = ms;
+    c->launches++;
+  }
+  if (e0) cudaEventDestroy(e0);
+  if (e1) cudaEventDestroy(e1);
+  cudaFree(sink);
+  if (e != cudaSuccess) return fail_cuda(c, e, "fp64 peak");
+  const double n = (double)blocks * kDfmaThreads * kDfmaChains * kDfmaUnroll * (double)iters;
+  *dfma_per_s = n / ((double)best * 1e-3);
   return CARDIAC_OK;
 }
 

@@ -19,12 +19,10 @@ cudaError_t pair_run(const Problem& pb, const PairLaunch& pl, cudaStream_t strea
   using PG = PairTile;
   using S = PairShape<MD, STENCIL, PG>;
   auto kern = pair_kernel<MD, STENCIL, KA, KB, STORE_MID, PG>;
-  static bool configured = false;  // per instantiation
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  static PerDeviceOnce configured;  // per instantiation and device
+  cudaError_t ec = configured.run(
+      [&] { return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, S::SMEM_BYTES); });
+  if (ec != cudaSuccess) return ec;
   if (KB == K_RK4F && pl.B != pl.in) return cudaErrorInvalidValue;   // Y3 is read as substep A's input
   PairArgs<MD> a;
   // unused operands alias valid buffers so that every pointer the kernel forms is valid

@@ -3,7 +3,29 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <atomic>
+
 namespace cardiac {
+
+// Function attributes (dynamic shared memory limit, non-portable cluster size) and occupancy are per
+// DEVICE; a context captures the device it was created on (api.cu), so "done once" is kept per device:
+// bit d of the mask = done on device d.  Safe from several host threads (setting an attribute twice is
+// harmless; the bit is published after the call succeeded).
+struct PerDeviceOnce {
+  std::atomic<unsigned long long> mask{0};
+  template <class F>
+  cudaError_t run(F&& f) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return f();   // beyond the mask: configure every time
+    const unsigned long long bit = 1ull << dev;
+    if (mask.load(std::memory_order_acquire) & bit) return cudaSuccess;
+    if ((e = f()) != cudaSuccess) return e;
+    mask.fetch_or(bit, std::memory_order_release);
+    return cudaSuccess;
+  }
+};
 
 struct Problem {
   int model, stencil, integrator, boundary, variant;
@@ -101,6 +123,7 @@ struct ResidentShape {
   int slab;    // rows per CTA
   size_t smem; // dynamic shared memory per CTA
 };
+constexpr size_t kResidentMaxSmem = 200 * 1024;   // per CTA
 inline ResidentShape resident_shape(const Problem& pb) {
   ResidentShape rs{0, 0, 0};
   if (pb.integrator > 2 || pb.nz > 1) return rs;  // Euler, Heun, RK4; 2-D
@@ -112,7 +135,7 @@ inline ResidentShape resident_shape(const Problem& pb) {
     const size_t smem = 2 * (size_t)pb.nd * sp * ((size_t)slab + 2 * pb.radius) * sizeof(double);
     // fits, and one cell per thread where the grid is large enough to spread (a substep costs the
     // barrier plus the latency of one warp's instruction sequence, resident.cuh CPT)
-    if (npx * slab <= cap && smem <= 200 * 1024 && (c == cmax || (pb.ny + 2 * c - 1) / (2 * c) < 4)) {
+    if (npx * slab <= cap && smem <= kResidentMaxSmem && (c == cmax || (pb.ny + 2 * c - 1) / (2 * c) < 4)) {
       rs.csize = c; rs.slab = slab; rs.smem = smem;
       return rs;
     }
@@ -149,5 +172,11 @@ inline cudaError_t launch_resident(const Problem& pb, const ResidentLaunch& rl, 
 enum { PROBE_EXP = 0, PROBE_RCP = 1, PROBE_HK = 2, PROBE_REACTION = 3 };
 cudaError_t launch_probe(const Problem& pb, int what, const double* in, double* out, long long n,
                          cudaStream_t stream);
+
+
+// FP64-pipe microbenchmark (cardiac_measure_fp64_peak): `blocks` CTAs of kDfmaThreads threads, each thread
+// kDfmaChains independent chains of iters x kDfmaUnroll DFMAs; one double per thread is stored to `sink`
+constexpr int kDfmaThreads = 256, kDfmaChains = 8, kDfmaUnroll = 64;
+cudaError_t launch_dfma_peak(double* sink, int blocks, int iters, cudaStream_t stream);
 
 }  // namespace cardiac

@@ -38,7 +38,28 @@ cudaError_t run_reaction(const Problem& pb, const double* z, double* f, long lon
   return cudaGetLastError();
 }
 
+// FP64-pipe microbenchmark: 8 independent DFMA chains per thread, registers only.  The result is
+// stored so that the chains stay live; x stays bounded (|a| < 1: x -> a x + b converges).
+__global__ void __launch_bounds__(256, 4) dfma_peak_kernel(double* __restrict__ sink, int iters, double a, double b) {
+  double x0 = threadIdx.x * 1e-3, x1 = x0 + 0.1, x2 = x0 + 0.2, x3 = x0 + 0.3, x4 = x0 + 0.4, x5 = x0 + 0.5,
+         x6 = x0 + 0.6, x7 = x0 + 0.7;
+#pragma unroll 1
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int k = 0; k < 64; ++k) {
+      x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+      x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+  }
+  sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+}
+
 }  // namespace
+
+cudaError_t launch_dfma_peak(double* sink, int blocks, int iters, cudaStream_t s) {
+  dfma_peak_kernel<<<blocks, kDfmaThreads, 0, s>>>(sink, iters, 0.999999, 1e-7);
+  return cudaGetLastError();
+}
 
 cudaError_t launch_probe(const Problem& pb, int what, const double* in, double* out, long long n,
                          cudaStream_t s) {

@@ -45,18 +45,14 @@ cudaError_t resident_run(const Problem& pb, const ResidentLaunch& rl, cudaStream
   for (int q = 0; q < MD::ND; ++q) a.lapw[q] = a.p.D[q] * stencil_norm(STENCIL) / (pb.dx * pb.dx);
   const size_t smem = rs.smem;
   if ((long long)a.npx * rs.slab * (3 - CPT) > (long long)kResidentThreads * KP) return cudaErrorInvalidValue;
-  static bool nonportable = false;
-  if (rs.csize > 8 && !nonportable) {
+  // per instantiation and device: clusters of 16 CTAs, and the largest slab resident_shape() ever asks for
+  static PerDeviceOnce configured;
+  cudaError_t ec = configured.run([&] {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
     if (e != cudaSuccess) return e;
-    nonportable = true;
-  }
-  static size_t configured = 0;  // per instantiation
-  if (smem > configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    configured = smem;
-  }
+    return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kResidentMaxSmem);
+  });
+  if (ec != cudaSuccess) return ec;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)pb.batch * rs.csize);
   cfg.blockDim = dim3(kResidentThreads);

@@ -24,6 +24,7 @@
 #include <cuda.h>   // CUtensorMap and its enums only; the encoder is fetched at run time (no -lcuda)
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cstdint>
 #include <cstring>
 #include <mutex>
@@ -336,18 +337,25 @@ template <class MD, int STENCIL, int KIND>
 cudaError_t run_ring(const Problem& pb, const StageLaunch& st, cudaStream_t stream) {
   using L = SlotLayout<MD, STENCIL, KIND>;
   auto kern = ring_stage_kernel<MD, STENCIL, KIND>;
-  static int ctas_per_sm = 0, num_sms = 0;   // per instantiation
-  if (ctas_per_sm == 0) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, L::SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    int dev = 0, occ = 0;
-    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
-    if ((e = cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, NTHREADS, L::SMEM_BYTES)) != cudaSuccess)
-      return e;
+  // per instantiation and device: the shared-memory limit, and the size of the persistent grid
+  static PerDeviceOnce configured;
+  static std::atomic<int> grid_of[64];
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+  e = configured.run([&] {
+    cudaError_t e2 = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, L::SMEM_BYTES);
+    if (e2 != cudaSuccess) return e2;
+    int sms = 0, occ = 0;
+    if ((e2 = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e2;
+    if ((e2 = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, NTHREADS, L::SMEM_BYTES)) != cudaSuccess)
+      return e2;
     if (occ < 1) return cudaErrorLaunchOutOfResources;
-    ctas_per_sm = occ;
-  }
+    grid_of[dev].store(sms * occ, std::memory_order_relaxed);
+    return cudaSuccess;
+  });
+  if (e != cudaSuccess) return e;
   RingArgs<MD> ra;
   StageArgs<MD>& a = ra.a;
   a.in = st.in; a.y = st.y ? st.y : st.in; a.A = st.A ? st.A : st.in; a.B = st.B ? st.B : st.in;
@@ -368,7 +376,6 @@ cudaError_t run_ring(const Problem& pb, const StageLaunch& st, cudaStream_t stre
   ra.per_row = make_fastdiv((unsigned)tiles_x);
 
   CUtensorMap tm_halo, tm_gate, tm_y, tm_A, tm_B;
-  cudaError_t e;
   if ((e = tensor_map(a.in, pb, MD::ND, HP, L::HR, &tm_halo)) != cudaSuccess) return e;
   tm_gate = tm_halo;
   if (L::NG > 0 &&
@@ -380,7 +387,7 @@ cudaError_t run_ring(const Problem& pb, const StageLaunch& st, cudaStream_t stre
     if ((e = tensor_map(a.A, pb, MD::NV, TW, TH, &tm_A)) != cudaSuccess) return e;
     if ((e = tensor_map(a.B, pb, MD::NV, TW, TH, &tm_B)) != cudaSuccess) return e;
   }
-  long long grid = (long long)num_sms * ctas_per_sm;
+  long long grid = grid_of[dev].load(std::memory_order_relaxed);
   if (grid > ra.ntiles) grid = ra.ntiles;
   kern<<<(unsigned)grid, NTHREADS, L::SMEM_BYTES, stream>>>(ra, tm_halo, tm_gate, tm_y, tm_A, tm_B);
   return cudaGetLastError();

@@ -79,12 +79,10 @@ cudaError_t fused_run(const Problem& pb, const TileLaunch& tl, cudaStream_t stre
   using TG = typename FusedGeom<MD, H, WIN>::type;
   using E = TileEngine<MD, STENCIL, INTEG, KSTEPS, TG>;
   auto kern = fused_step_kernel<MD, STENCIL, INTEG, KSTEPS, TG>;
-  static bool configured = false;  // per instantiation
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, E::SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  static PerDeviceOnce configured;  // per instantiation and device
+  cudaError_t ec = configured.run(
+      [&] { return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, E::SMEM_BYTES); });
+  if (ec != cudaSuccess) return ec;
   TileArgs<MD> a;
   fill_tile_args<MD>(pb, STENCIL, a);
   a.in = tl.in; a.out = tl.out;

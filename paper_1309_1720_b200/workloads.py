@@ -227,6 +227,14 @@ def stimulus_cfg4(state: np.ndarray) -> np.ndarray:
     return out
 
 
+def stimulus_cfg4_inplace(state):
+    """The same edit in place on a numpy array or a torch tensor (host or device): plain slice
+    assignment, no arithmetic."""
+    ny = state.shape[-2]
+    state[:, 0, : ny // 2, :] = 1.0
+    return state
+
+
 def directions_cfg5(cfg: Config, nvec: int, seed: int | None = None) -> np.ndarray:
     """nvec Gaussian directions over all n_v*ny*nx entries, Euclidean norm 1 each."""
     seed = cfg.seed if seed is None else seed
@@ -246,9 +254,24 @@ def state_cfg5(cfg: Config, base: np.ndarray, eps: float = 1e-7) -> np.ndarray:
     return z
 
 
+CFG5_BASE_STEPS = 5_000
+
+
+def base_recipe_cfg5(cfg: Config) -> tuple[Config, np.ndarray, int]:
+    """What BASELINE.json:configs[4] defines the base of config 5 as: the config-2-shaped state
+    (same grid as `cfg`, seed 2) after 5,000 RK4 steps.  Returns (single-member config, its initial
+    state, number of steps); the CALLER integrates it — with the oracle in tests/ and in
+    bench.py --impl reference, with the library in bench.py — because this module holds none of the
+    method's arithmetic — and passes the result to initial_state(cfg, base=...)."""
+    one = replace(cfg, batch=1, nsteps=CFG5_BASE_STEPS, name="cfg2" if "@" not in cfg.name else f"cfg2@{cfg.nx}",
+                  seed=2)
+    return one, state_cfg2(one), CFG5_BASE_STEPS
+
+
 def synthetic_base_cfg5(cfg: Config) -> np.ndarray:
-    """Stand-in for 'config-2 state after 5000 steps' where running 5000 steps is not the point
-    (parity cases): the config-2 initial state blurred so it is smooth like an evolved state."""
+    """Stand-in for 'config-2 state after 5000 steps' for the SCALED parity cases only (cfg5@N, where
+    running 5000 steps is not the point): the config-2 initial state blurred so it is smooth like an
+    evolved state.  The full-size config 5 never uses it (initial_state insists on a real base)."""
     one = replace(cfg, batch=1)
     z = state_cfg2(one, noise=0.0)[0]
     for f in range(z.shape[0]):
@@ -300,21 +323,27 @@ def default_dt_3d(model: int) -> float:
     return 0.5 * DX[model] ** 2 / (6.0 * D_MAX[model])
 
 
-def initial_state(cfg: Config) -> np.ndarray:
-    """Initial state of a (possibly scaled) baseline config, dense [batch][n_v][ny][nx]."""
+def initial_state(cfg: Config, base: np.ndarray | None = None) -> np.ndarray:
+    """Initial state of a (possibly scaled) baseline config, dense [batch][n_v][ny][nx].
+    Config 5 at full size needs `base`, the integrated state of base_recipe_cfg5()."""
     if cfg.nz > 1:
         return state_3d(cfg)
-    base = cfg.name.split("@")[0]
-    if base == "cfg1":
+    name = cfg.name.split("@")[0]
+    if name == "cfg1":
         return state_cfg1(cfg)
-    if base == "cfg2":
+    if name == "cfg2":
         return state_cfg2(cfg)
-    if base == "cfg3":
+    if name == "cfg3":
         return state_blocks(cfg)
-    if base == "cfg4":
+    if name == "cfg4":
         return state_cfg4(cfg)
-    if base == "cfg5":
-        return state_cfg5(cfg, synthetic_base_cfg5(cfg))
+    if name == "cfg5":
+        if base is None:
+            if "@" not in cfg.name:
+                raise ValueError("config 5 is defined on the config-2 state after 5000 RK4 steps: integrate "
+                                 "base_recipe_cfg5(cfg) and pass it as base=")
+            base = synthetic_base_cfg5(cfg)
+        return state_cfg5(cfg, base)
     z = state_blocks(cfg)
     if cfg.batch > 1:
         z = np.repeat(z, cfg.batch, axis=0)

@@ -18,10 +18,10 @@ def C():
     return cardiac
 
 
-def _declared_functions():
-    src = open(os.path.join(ROOT, "include", "cardiac.h")).read()
+def _declared_functions(header="cardiac.h"):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(cardiac_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(cardiac_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_every_declared_symbol_is_exported(C):
@@ -33,6 +33,13 @@ def test_every_declared_symbol_is_exported(C):
     assert sorted(C.EXPORTS) == names           # the binding covers exactly the header
     for n in names:
         assert callable(getattr(C, n))          # same names in Python
+    # the diagnostics live in their own header (not part of the product boundary) and are covered likewise
+    diag = _declared_functions("cardiac_diag.h")
+    assert diag and not set(diag) & set(names)
+    assert sorted(C.DIAG_EXPORTS) == diag
+    for n in diag:
+        assert hasattr(lib, n) and callable(getattr(C, n))
+    assert not any(n in names for n in ("cardiac_probe", "cardiac_time_steps", "cardiac_launch_count"))
 
 
 def test_model_tables_and_defaults_agree_with_oracle(C):

@@ -12,6 +12,11 @@ from paper_1309_1720_b200 import workloads as W
 pytestmark = pytest.mark.gpu
 
 TOL_1, TOL_100 = 1e-12, 1e-9
+
+
+def tol(nsteps):
+    """1e-12 at one step, 1e-9 at 100 (north_star), linear in between: TOL_1 x 10 x nsteps."""
+    return TOL_1 if nsteps <= 1 else min(TOL_100, TOL_1 * 10 * nsteps)
 FHN, KARMA, BOCF = W.FHN, W.KARMA, W.BOCF
 LAP5, LAP9X4, BOX9 = W.LAP5, W.LAP9X4, W.BOX9
 EULER, HEUN, RK4, RL, IE = W.EULER, W.HEUN, W.RK4, W.RUSH_LARSEN, W.IMPLICIT_EULER
@@ -59,7 +64,7 @@ def test_parity_3d_one_and_fifty_steps(C, model, stencil, integ):
     got = gpu_run(C, cfg, Z, 50)
     ref = O.step3d(model, ref1, cfg.dx, cfg.dt, cfg.scheme, 49, omp=True)
     assert np.all(np.isfinite(got))
-    assert maxabs(got, ref) <= TOL_100
+    assert maxabs(got, ref) <= tol(50)
     assert maxabs(got, Z) > 1e-6
 
 
@@ -71,14 +76,14 @@ def test_parity_3d_edges_and_periodic(C, model, stencil, nx, ny, nz, bc):
     cfg, Z = make(model, nx, ny, nz, stencil, RK4, boundary=bc)
     got = gpu_run(C, cfg, Z, 20)
     ref = O.step3d(model, Z, cfg.dx, cfg.dt, cfg.scheme, 20)
-    assert maxabs(got, ref) <= TOL_100
+    assert maxabs(got, ref) <= tol(20)
 
 
 def test_3d_batch_jvp_and_composition(C):
     cfg, Z = make(FHN, 70, 20, 6, LAP9X4, RK4, batch=4, seed=2)
     got = gpu_run(C, cfg, Z, 12)
     ref = O.step3d(FHN, Z, cfg.dx, cfg.dt, cfg.scheme, 12)
-    assert maxabs(got, ref) <= TOL_100
+    assert maxabs(got, ref) <= tol(12)
     perm = [2, 0, 3, 1]
     assert np.array_equal(gpu_run(C, cfg, Z[perm], 12), got[perm])          # whatever the slot
     assert np.array_equal(gpu_run(C, cfg, Z, 12, chunks=[1, 5, 6]), got)     # step(a); step(b) == step(a+b)

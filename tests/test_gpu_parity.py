@@ -14,6 +14,13 @@ pytestmark = pytest.mark.gpu
 TOL_1 = 1e-12     # one step
 TOL_100 = 1e-9    # 100 steps
 
+
+def tol(nsteps):
+    """Tolerance after `nsteps` steps: north_star fixes 1e-12 at one step and 1e-9 at 100; in between the
+    bound grows linearly, TOL_1 x 10 x nsteps (= TOL_100 at 100 steps), so that a 20-step case is held to
+    2e-10 and not to the 100-step bound (measured <= 2e-13 after 100 steps)."""
+    return TOL_1 if nsteps <= 1 else min(TOL_100, TOL_1 * 10 * nsteps)
+
 FHN, KARMA, BOCF = W.FHN, W.KARMA, W.BOCF
 LAP5, LAP9X4, BOX9 = W.LAP5, W.LAP9X4, W.BOX9
 EULER, HEUN, RK4, RL, IE = W.EULER, W.HEUN, W.RK4, W.RUSH_LARSEN, W.IMPLICIT_EULER
@@ -86,7 +93,7 @@ def test_parity_fused_small_window(C, model, stencil, integ):
     cfg, Z = make(model, 150, 97, stencil, integ, seed=5)
     small = gpu_run(C, cfg, Z, 40, plan=(2, 2))
     ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 40)
-    assert maxabs(small, ref) <= TOL_100
+    assert maxabs(small, ref) <= tol(40)
     large = gpu_run(C, cfg, Z, 40, plan=(2, 1))
     assert maxabs(small, large) <= 1e-12
     auto = gpu_run(C, cfg, Z, 40, plan=(2, 0))
@@ -94,7 +101,7 @@ def test_parity_fused_small_window(C, model, stencil, integ):
     if integ == RK4:          # the three other one-CTA-per-SM windows, several ragged tiles each
         for win in (3, 4, 5):
             other = gpu_run(C, cfg, Z, 40, plan=(2, win))
-            assert maxabs(other, ref) <= TOL_100 and maxabs(other, large) <= 1e-12
+            assert maxabs(other, ref) <= tol(40) and maxabs(other, large) <= 1e-12
     else:
         with C.Context.from_config(cfg, plan=2) as ctx:
             with pytest.raises(C.CardiacError):
@@ -140,7 +147,7 @@ def test_parity_persistent_edges(C, model, stencil, nx, ny, bc):
     cfg, Z = make(model, nx, ny, stencil, RK4, boundary=bc)
     got = gpu_run(C, cfg, Z, 30, plan=PERSISTENT)
     ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 30)
-    assert maxabs(got, ref) <= TOL_100
+    assert maxabs(got, ref) <= tol(30)
 
 
 @pytest.mark.parametrize("model,stencil,integ,n,batch,nsteps", [(FHN, LAP5, EULER, 64, 1, 6000), (KARMA, LAP9X4, RK4, 96, 4, 1500),
@@ -208,7 +215,7 @@ def test_parity_periodic_boundary(C, model, stencil, integ, plan):
     cfg, Z = make(model, 37, 50, stencil, integ, boundary=1)
     got = gpu_run(C, cfg, Z, 30, plan=plan)
     ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 30)
-    assert maxabs(got, ref) <= TOL_100
+    assert maxabs(got, ref) <= tol(30)
 
 
 @pytest.mark.parametrize("model", [KARMA, BOCF])
@@ -217,7 +224,7 @@ def test_parity_tanhfree_variant(C, model, plan):
     cfg, Z = make(model, 40, 33, LAP9X4, RK4, variant=1)
     got = gpu_run(C, cfg, Z, 50, plan=plan)
     ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 50)
-    assert maxabs(got, ref) <= TOL_100
+    assert maxabs(got, ref) <= tol(50)
     ref_paper = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme & 0xFFFFFF, 50)
     assert maxabs(ref, ref_paper) > 1e-6   # the variant really is a different model
 
@@ -231,7 +238,7 @@ def test_parity_degenerate_sizes(C, model, stencil, nx, ny, plan):
     cfg, Z = make(model, nx, ny, stencil, RK4)
     got = gpu_run(C, cfg, Z, 20, plan=plan)
     ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 20)
-    assert maxabs(got, ref) <= TOL_100
+    assert maxabs(got, ref) <= tol(20)
 
 
 @pytest.mark.parametrize("plan", [STAGE, RING, FUSED, PAIR])
@@ -241,7 +248,7 @@ def test_batch_members_independent_of_position(C, plan):
         return gpu_run(C, cfg, Z, n, plan=plan)
     got = gpu_run_p(C, cfg, Z, 10)
     ref = O.step(KARMA, Z, cfg.dx, cfg.dt, cfg.scheme, 10)
-    assert maxabs(got, ref) <= TOL_100
+    assert maxabs(got, ref) <= tol(10)
     perm = [3, 0, 4, 2, 1]
     got_p = gpu_run_p(C, cfg, Z[perm], 10)
     assert np.array_equal(got_p, got[perm])                 # bitwise, whatever the slot
@@ -273,7 +280,7 @@ def test_fused_many_tiles_matches_stage_plan_and_oracle(C):
         cfg, Z = make(model, 250, 170, stencil, integ, seed=21)
         got = gpu_run(C, cfg, Z, 12, plan=FUSED)
         ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 12)
-        assert maxabs(got, ref) <= TOL_100
+        assert maxabs(got, ref) <= tol(12)
         direct = gpu_run(C, cfg, Z, 12, plan=STAGE)
         assert maxabs(got, direct) <= 1e-12
         # the TMA-ring kernels run the same arithmetic per cell as the direct ones: bitwise equal
@@ -291,7 +298,7 @@ def test_pair_plan_many_tiles_bitwise_equal_to_stage_plan(C, model, stencil, int
     cfg, Z = make(model, 251, 170, stencil, integ, seed=21, boundary=bc, batch=2)
     got = gpu_run(C, cfg, Z, 13, plan=PAIR)
     ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 13)
-    assert maxabs(got, ref) <= TOL_100
+    assert maxabs(got, ref) <= tol(13)
     assert np.array_equal(got, gpu_run(C, cfg, Z, 13, plan=STAGE))
 
 
@@ -305,7 +312,7 @@ def test_pair_plan_tile_edges(C, nx, ny, stencil, bc):
     cfg, Z = make(BOCF, nx, ny, stencil, RK4, seed=nx * 131 + ny, boundary=bc)
     got = gpu_run(C, cfg, Z, 3, plan=PAIR)
     assert np.array_equal(got, gpu_run(C, cfg, Z, 3, plan=STAGE))
-    assert maxabs(got, O.step(BOCF, Z, cfg.dx, cfg.dt, cfg.scheme, 3)) <= TOL_100
+    assert maxabs(got, O.step(BOCF, Z, cfg.dx, cfg.dt, cfg.scheme, 3)) <= tol(3)
 
 
 def test_pair_plan_limits(C):
@@ -353,7 +360,7 @@ def test_plan_switch_keeps_state(C):
         C.cardiac_set_plan(ctx.ctx, *STAGE)
         ctx.step(1)
         got = ctx.get_state()
-    assert maxabs(got, O.step(FHN, Z, cfg.dx, cfg.dt, cfg.scheme, 15)) <= TOL_100
+    assert maxabs(got, O.step(FHN, Z, cfg.dx, cfg.dt, cfg.scheme, 15)) <= tol(15)
 
 
 def test_uniform_state_and_rest_state(C):
@@ -380,7 +387,7 @@ def test_custom_parameters(C):
     p[0], p[1], p[5], p[7] = 0.002, 3.0, 1.4, 4.0          # gamma, tau_u, u_star, M = 4
     got = gpu_run(C, cfg, Z, 20, params=p)
     ref = O.step(KARMA, Z, cfg.dx, cfg.dt, cfg.scheme, 20, params=p)
-    assert maxabs(got, ref) <= TOL_100
+    assert maxabs(got, ref) <= tol(20)
     assert maxabs(ref, O.step(KARMA, Z, cfg.dx, cfg.dt, cfg.scheme, 20)) > 1e-4
     with C.Context.from_config(cfg) as ctx:
         C.cardiac_set_params(ctx.ctx, p)
@@ -422,7 +429,7 @@ def test_error_paths_and_device_buffers(C):
         C.cardiac_get_state(ctx, od)
         torch.cuda.synchronize()
         ref = O.step(FHN, Z, cfg.dx, cfg.dt, cfg.scheme, 5)
-        assert maxabs(od.cpu().numpy(), ref) <= TOL_100
+        assert maxabs(od.cpu().numpy(), ref) <= tol(5)
         assert C.cardiac_launch_count(ctx) == 5
         with pytest.raises(C.CardiacError):
             C.cardiac_set_plan(ctx, 99, 0)
@@ -447,7 +454,7 @@ def test_non_default_stream(C):
             ctx.get_state(od)
             s.synchronize()
     ref = O.step(FHN, Z, cfg.dx, cfg.dt, cfg.scheme, 40)
-    assert maxabs(od.cpu().numpy(), ref) <= TOL_100
+    assert maxabs(od.cpu().numpy(), ref) <= tol(40)
 
 
 # ----------------------------------------------------------------------------- the BASELINE configs at full size
@@ -460,22 +467,28 @@ def test_config1_full(C):
     assert maxabs(gpu_run(C, cfg, Z, 1), O.step(cfg.model, Z, cfg.dx, cfg.dt, cfg.scheme, 1)) <= TOL_1
 
 
-@pytest.mark.parametrize("idx,n100,omp", [(2, 100, False), (3, 100, True), (4, 25, True)])
-def test_configs_full_size_step1_and_step100(C, idx, n100, omp):
-    """Full-size grids, in the launch configuration bench.py times; for the large grids the oracle
-    runs its -fopenmp build (independent loops split over threads, bitwise the same numbers), and
-    config 4 (4.2 M cells x 4 fields of the exp-heavy model) stops at 25 steps to bound CPU time."""
+@pytest.mark.parametrize("idx,omp", [(2, False), (3, True), (4, True)])
+def test_configs_full_size_step1_and_step100(C, idx, omp):
+    """Full-size grids, in the launch configuration bench.py times (AUTO plan; the 99 steps are ONE
+    cardiac_step call, so the CUDA graph of the plan — 60 kernel nodes = 30 time steps of config 4's plan
+    PAIR — replays at full size, followed by its remainder of direct launches); for the large grids the
+    oracle runs its -fopenmp build (independent loops split over threads, bitwise the same numbers)."""
     cfg = W.baseline_config(idx)
     Z = W.initial_state(cfg)
     with C.Context.from_config(cfg) as ctx:
+        if idx == 4:
+            assert ctx.plan == PAIR
         ctx.set_state(Z)
         ctx.step(1)
         got1 = ctx.get_state()
-        ctx.step(n100 - 1)
+        l0 = ctx.launches
+        ctx.step(99)
+        if idx == 4:
+            assert ctx.launches - l0 == 2 * 99          # two launches per RK4 step, graph + remainder
         got = ctx.get_state()
     ref1 = O.step(cfg.model, Z, cfg.dx, cfg.dt, cfg.scheme, 1, omp=omp)
     assert maxabs(got1, ref1) <= TOL_1
-    ref = O.step(cfg.model, ref1, cfg.dx, cfg.dt, cfg.scheme, n100 - 1, omp=omp)
+    ref = O.step(cfg.model, ref1, cfg.dx, cfg.dt, cfg.scheme, 99, omp=omp)
     assert maxabs(got, ref) <= TOL_100
 
 
@@ -495,13 +508,52 @@ def test_config4_stimulus_path(C):
     assert maxabs(got, ref) <= TOL_100
 
 
-def test_config5_jvp_full_size(C):
-    """17 x 512^2 in one batched launch; states at the state tolerance, JVPs at 1e-6 absolute
-    (= 1e-13/eps, Q16)."""
+def test_config4_stimulus_path_full_size(C):
+    """The same at 2048^2 in the plan bench.py times (PAIR, graph replay on both sides of the stimulus):
+    30 steps, the cross-field stimulus through get_state / host edit / set_state, 30 more steps."""
+    cfg = W.baseline_config(4)
+    Z = W.initial_state(cfg)
+    with C.Context.from_config(cfg) as ctx:
+        ctx.set_state(Z)
+        ctx.step(30)
+        mid = W.stimulus_cfg4(ctx.get_state())
+        ctx.set_state(mid)
+        ctx.step(30)
+        got = ctx.get_state()
+    ref_mid = W.stimulus_cfg4(O.step(BOCF, Z, cfg.dx, cfg.dt, cfg.scheme, 30, omp=True))
+    assert maxabs(mid, ref_mid) <= tol(30)
+    ref = O.step(BOCF, ref_mid, cfg.dx, cfg.dt, cfg.scheme, 30, omp=True)
+    assert maxabs(got, ref) <= tol(60)
+    assert maxabs(got[:, 0, :1024], 1.0) < 1.0 and maxabs(got, mid) > 1e-3      # the stimulated half is evolving
+
+
+@pytest.fixture(scope="module")
+def cfg5_base():
+    """BASELINE.json:configs[4]: the config-2 state after 5,000 RK4 steps — integrated by the ORACLE
+    (OpenMP build, same arithmetic), never by the CUDA path."""
+    one, z2, n = W.base_recipe_cfg5(W.baseline_config(5))
+    return O.step(one.model, z2, one.dx, one.dt, one.scheme, n, omp=True)[0]
+
+
+def test_config5_base_is_the_evolved_config2_state(C, cfg5_base):
+    """The base is far from the initial state (the wave front has moved), finite and inside the printed
+    range; the CUDA path integrated over the same 5,000 steps lands on it (not chaotic on this horizon:
+    roundoff differences stay at roundoff)."""
+    cfg2 = W.baseline_config(2)
+    z2 = W.initial_state(cfg2)
+    assert np.isfinite(cfg5_base).all() and maxabs(cfg5_base, z2[0]) > 0.1
+    assert -1.3 < cfg5_base[0].min() and cfg5_base[0].max() < 1.3
+    got = gpu_run(C, cfg2, z2, W.CFG5_BASE_STEPS)
+    assert maxabs(got[0], cfg5_base) <= 1e-8
+
+
+def test_config5_jvp_full_size(C, cfg5_base):
+    """17 x 512^2 in one batched launch from the real base state, 100 steps; states at the state
+    tolerance, JVPs at 1e-6 absolute (= 1e-13/eps, Q16)."""
     cfg = W.baseline_config(5)
     eps = 1e-7
-    Z = W.initial_state(cfg)
-    n = 20
+    Z = W.initial_state(cfg, base=cfg5_base)
+    n = 100
     with C.Context.from_config(cfg) as ctx:
         ctx.set_state(Z)
         ctx.step(n)
@@ -511,7 +563,9 @@ def test_config5_jvp_full_size(C):
         Jd = torch.empty(J.shape, dtype=torch.float64, device="cuda")
         ctx.get_jvp(eps, Jd)
         torch.cuda.synchronize()
+        again = ctx.get_state()
     assert np.array_equal(Jd.cpu().numpy(), J)
+    assert np.array_equal(again, got)                       # the host-side JVP staged in a free stage buffer
     ref = O.step(cfg.model, Z, cfg.dx, cfg.dt, cfg.scheme, n, omp=True)
     assert maxabs(got, ref) <= TOL_100
     assert np.array_equal(J, (got[1:] - got[0]) / eps)     # exactly the FD quotient of the states

@@ -75,7 +75,51 @@ def test_slabs_equal_single_grid_bitwise(C, model, stencil, integ, plan, bc, wor
         ctx.step(nsteps)
         whole = ctx.get_state()
     assert np.array_equal(got, whole)
-    assert float(np.max(np.abs(got - O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, nsteps)))) <= 1e-9
+    assert float(np.max(np.abs(got - O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, nsteps)))) <= 1e-12 * 10 * nsteps
+
+
+def test_get_rows_writes_straight_into_another_contexts_memory(C):
+    """include/cardiac.h: a DEVICE destination of cardiac_get_rows may be any address the GPU can store
+    to — e.g. a peer's buffer mapped over NVLink, so that the pack kernel IS the transfer.  One GPU here:
+    the destination is memory owned by ANOTHER context's caller-provided workspace region (as a peer's
+    receive buffer would be), written by the sender's pack kernel on the sender's stream, consumed by
+    the receiver's set_rows on ITS stream after an event — no host copy, no staging, no NCCL."""
+    import torch
+    cfg = W.make_config("peer", W.FHN, 70, W.LAP9X4, W.RK4, 0, batch=2, seed=9, ny=64)
+    Z = W.initial_state(cfg)
+    g = D.ghost_depth(2, 4)                                     # 8 ghost rows per cut
+    slabs = [D.slab_of(cfg.ny, r, 2, g) for r in range(2)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    ctxs, inbox = [], []
+    for s, st in zip(slabs, streams):
+        with torch.cuda.stream(st):
+            c = C.Context(cfg.model, cfg.nx, s.ext_rows, cfg.dx, cfg.dt, cfg.scheme, cfg.batch)
+            c.set_state(np.ascontiguousarray(Z[:, :, s.global_rows(), :]))
+            # the receive buffer lives next to the receiver's workspace, in the receiver's allocation
+            inbox.append(torch.empty((cfg.batch, cfg.n_v, g, cfg.nx), dtype=torch.float64, device="cuda"))
+            ctxs.append(c)
+    torch.cuda.synchronize()
+    for step in range(6):
+        done = []
+        for r, (c, st) in enumerate(zip(ctxs, streams)):
+            with torch.cuda.stream(st):
+                c.step(1)
+                # own rows next to the cut -> the OTHER context's inbox
+                j0, n = slabs[r].send_to_upper() if r == 0 else slabs[r].send_to_lower()
+                c.get_rows(j0, n, inbox[1 - r])
+                ev = torch.cuda.Event(); ev.record(st); done.append(ev)
+        for r, (c, st) in enumerate(zip(ctxs, streams)):
+            with torch.cuda.stream(st):
+                st.wait_event(done[1 - r])
+                c.set_rows((slabs[r].recv_from_upper() if r == 0 else slabs[r].recv_from_lower())[0], inbox[r])
+        torch.cuda.synchronize()
+    got = np.concatenate([c.get_rows(s.g_lo, s.own) for c, s in zip(ctxs, slabs)], axis=2)
+    for c in ctxs:
+        c.close()
+    with C.Context.from_config(cfg) as ctx:
+        ctx.set_state(Z); ctx.step(6)
+        whole = ctx.get_state()
+    assert np.array_equal(got, whole)
 
 
 def test_rows_roundtrip_and_errors(C):

@@ -66,6 +66,15 @@ def test_initial_states():
     d = (z[1:] - z[0]) / 1e-7
     assert np.allclose(np.sqrt(np.sum(d ** 2, axis=(1, 2, 3))), 1.0, atol=1e-6)
     assert abs(np.sum(d[0] * d[1])) < 0.2                 # different directions
+    # full size: the base is BASELINE.json:configs[4]'s "config-2 state after 5000 RK4 steps", never a stand-in
+    c5f = W.baseline_config(5)
+    with pytest.raises(ValueError):
+        W.initial_state(c5f)
+    one, z2, n = W.base_recipe_cfg5(c5f)
+    assert n == 5000 and (one.batch, one.nx, one.ny, one.integrator, one.stencil) == (1, 512, 512, W.RK4, W.LAP9X4)
+    assert np.array_equal(z2, W.initial_state(W.baseline_config(2)))
+    zf = W.initial_state(c5f, base=z2[0])
+    assert zf.shape == (17, 2, 512, 512) and np.array_equal(zf[0], z2[0])
 
 
 def test_sweep_and_3d_inputs():

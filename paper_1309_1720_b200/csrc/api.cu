@@ -151,11 +151,69 @@ int enqueue_fused(cardiac_ctx* c, cudaStream_t s, int ksteps) {
   return CARDIAC_OK;
 }
 
+// Plan PAIR: which implementation runs (bitwise identical results): DIRECT (pair.cuh) or TMA (pairt.cuh)
+bool pair_uses_tma(const cardiac_ctx* c) {
+  const Problem& pb = c->pb;
+  if (pb.pair_impl == 1 || !pair_tma_supported(pb)) return false;
+  if (pb.pair_impl == 2) return true;
+  const long long ntiles = (long long)((pb.nx + 63) / 64) * ((pb.ny + 23) / 24) * pb.batch;
+  return ntiles >= kPairTMinTiles;
+}
+
+// ... TMA implementation: one time step (Heun, RK4) or two (Euler)
+int enqueue_pair_tma(cardiac_ctx* c, cudaStream_t s) {
+  const Problem& pb = c->pb;
+  const double dt = pb.dt;
+  const int ring = pb.integrator == I_RK4 ? 3 : 2;
+  const int n1 = c->cur < ring ? (c->cur + 1) % ring : 0, n2 = (n1 + 1) % ring;
+  double* b0 = c->buf[c->cur];
+  double* b1 = c->buf[n1];
+  auto go = [&](const PairTLaunch& pl) -> int {
+    cudaError_t e = launch_pairt(pb, pl, s);
+    if (e != cudaSuccess) return fail_cuda(c, e, "pair (TMA) launch");
+    c->launches++;
+    return CARDIAC_OK;
+  };
+  int rc = CARDIAC_OK;
+  PairTLaunch pl{};
+  pl.in = b0; pl.y = b0;
+  switch (pb.integrator) {
+    case I_EULER:
+      pl.ka = K_SELF; pl.kb = K_SELF; pl.out = b1; pl.a_wf = dt; pl.w_f = dt;
+      rc = go(pl);
+      break;
+    case I_HEUN:
+      pl.ka = K_SELF; pl.kb = K_BASE; pl.out = b1; pl.a_wf = dt;
+      pl.w_y = 0.5; pl.w_in = 0.5; pl.w_f = 0.5 * dt;
+      rc = go(pl);
+      break;
+    case I_RK4: {   // the combinations and weights of plan STAGE (enqueue_step); P takes Y2's place in memory
+      double* b2 = c->buf[n2];
+      pl.ka = K_SELF; pl.kb = K_BASE; pl.out = b2; pl.out2 = b1; pl.a_wf = 0.5 * dt;
+      pl.w_y = 1.0; pl.w_in = 0.0; pl.w_f = 0.5 * dt;
+      pl.p_wy = -1.0 / 3.0; pl.p_wA = 1.0 / 3.0; pl.p_wB = 2.0 / 3.0;
+      if ((rc = go(pl))) break;
+      pl = PairTLaunch{};
+      pl.ka = K_BASE; pl.kb = K_RK4F; pl.in = b2; pl.y = b0; pl.P = b1; pl.out = b1;
+      pl.a_wy = 1.0; pl.a_win = 0.0; pl.a_wf = dt;
+      pl.w_in = 1.0 / 3.0; pl.w_f = dt / 6.0;
+      rc = go(pl);
+      break;
+    }
+    default:
+      return fail(c, CARDIAC_ERR_INVALID, "PAIR supports Euler, Heun and RK4 only");
+  }
+  if (rc) return rc;
+  c->cur = n1;
+  return CARDIAC_OK;
+}
+
 // Plan PAIR: buffers the state rotates through (RK4: y, Y2, Y3 — Y4 never leaves the SM)
 int pair_ring(const cardiac_ctx* c) { return c->pb.integrator == I_RK4 ? 3 : 2; }
 
 // Plan PAIR: one time step (Heun, RK4) or two (Euler) in one or two launches of two substeps each.
 int enqueue_pair(cardiac_ctx* c, cudaStream_t s) {
+  if (pair_uses_tma(c)) return enqueue_pair_tma(c, s);
   const Problem& pb = c->pb;
   const double dt = pb.dt;
   const int ring = pair_ring(c);
@@ -477,7 +535,11 @@ int cardiac_set_plan(cardiac_ctx* c, int plan, int param) {
     }
   } else if (resolved == CARDIAC_PLAN_PAIR) {
     if (!rk_like) return fail(c, CARDIAC_ERR_INVALID, "PAIR supports Euler, Heun and RK4 only");
-    if (param != 0) return fail(c, CARDIAC_ERR_INVALID, "plan parameter must be 0");
+    if (param < 0 || param > 2)
+      return fail(c, CARDIAC_ERR_INVALID, "PAIR: parameter must be 0 (auto), 1 (direct) or 2 (TMA-fed persistent CTAs)");
+    if (param == 2 && !pair_tma_supported(c->pb))
+      return fail(c, CARDIAC_ERR_INVALID, "PAIR: the TMA implementation is not available for this context");
+    rparam = param;
   } else if (resolved == CARDIAC_PLAN_PERSISTENT) {
     if (!resident_supported(c->pb))
       return fail(c, CARDIAC_ERR_INVALID,
@@ -490,6 +552,7 @@ int cardiac_set_plan(cardiac_ctx* c, int plan, int param) {
   c->plan = resolved;
   c->plan_param = rparam;
   c->pb.stage_impl = resolved == CARDIAC_PLAN_STAGE ? rparam : 0;
+  c->pb.pair_impl = resolved == CARDIAC_PLAN_PAIR ? rparam : 0;
   drop_graphs(c);
   return CARDIAC_OK;
 }

@@ -37,6 +37,7 @@ struct Problem {
   double dx, dt;
   double params[32];    // public parameter block (include/cardiac.h)
   int stage_impl;       // plan STAGE: 0 = pick by size, 1 = DIRECT (stage_kernels.cu), 2 = RING (stream_kernels.cu)
+  int pair_impl;        // plan PAIR: 0 = pick by size, 1 = DIRECT (pair.cuh), 2 = TMA (pairt.cuh)
 };
 
 // One stage launch of the STAGE plan (kind = K_* of stage.cuh).
@@ -107,6 +108,32 @@ inline cudaError_t launch_pair(const Problem& pb, const PairLaunch& pl, cudaStre
   return pb.model == 0 ? launch_pair_fhn(pb, pl, stream)
                        : (pb.model == 1 ? launch_pair_karma(pb, pl, stream)
                                         : launch_pair_bocf(pb, pl, stream));
+}
+
+// pairt_kernels_*.cu: plan PAIR, implementation TMA (pairt.cuh) — the same two substeps per launch, persistent
+// CTAs fed by TMA box copies.  RK4: launch 1 (ka = K_SELF, kb = K_BASE, out = Y3, out2 = P), launch 2
+// (ka = K_BASE, kb = K_RK4F, in = Y3, y, P; out may be P's buffer).  out != in, out != y.
+struct PairTLaunch {
+  int ka, kb;
+  const double* in;
+  const double* y;
+  const double* P;
+  double* out;
+  double* out2;
+  double a_wy, a_win, a_wf;
+  double w_y, w_in, w_f;
+  double p_wy, p_wA, p_wB;
+};
+bool pair_tma_supported(const Problem& pb);   // 2-D, tensor maps available, fewer than 2^31 tiles
+// AUTO picks the TMA implementation once every persistent CTA has several tiles to pipeline
+constexpr long long kPairTMinTiles = 4 * 148;
+cudaError_t launch_pairt_fhn(const Problem& pb, const PairTLaunch& pl, cudaStream_t stream);
+cudaError_t launch_pairt_karma(const Problem& pb, const PairTLaunch& pl, cudaStream_t stream);
+cudaError_t launch_pairt_bocf(const Problem& pb, const PairTLaunch& pl, cudaStream_t stream);
+inline cudaError_t launch_pairt(const Problem& pb, const PairTLaunch& pl, cudaStream_t stream) {
+  return pb.model == 0 ? launch_pairt_fhn(pb, pl, stream)
+                       : (pb.model == 1 ? launch_pairt_karma(pb, pl, stream)
+                                        : launch_pairt_bocf(pb, pl, stream));
 }
 
 // resident_kernels_*.cu: plan PERSISTENT — one thread-block cluster of C <= 16 CTAs per batch member

@@ -21,7 +21,6 @@
 //
 // The arithmetic per cell is the one of stage_kernels.cu (same Stencil<>, Model<>::reaction,
 // combine<>), so both implementations give bitwise identical results.
-#include <cuda.h>   // CUtensorMap and its enums only; the encoder is fetched at run time (no -lcuda)
 #include <cuda_runtime.h>
 
 #include <atomic>
@@ -32,6 +31,7 @@
 
 #include "plans.h"
 #include "stage.cuh"
+#include "tma.cuh"
 
 namespace cardiac {
 
@@ -67,71 +67,17 @@ struct SlotLayout {
   static constexpr int SMEM_BYTES = NSLOT * SLOT_BYTES + 128;  // + the mbarriers
 };
 
-// n / d for n < 2^31 by one multiply-high and a shift (the round-up method of Granlund & Montgomery:
-// m = ceil(2^(31 + ceil(log2 d)) / d)); the tile loop would otherwise spend ~150 instructions per
-// tile on integer division, a third of the 4-field reaction itself
-struct FastDiv {
-  unsigned mul, shr, d;
-};
-FastDiv make_fastdiv(unsigned d) {
-  FastDiv f;
-  f.d = d;
-  unsigned lg = 0;
-  while ((1ull << lg) < d) ++lg;
-  f.mul = (unsigned)(((1ull << (31 + lg)) + d - 1) / d);
-  f.shr = lg == 0 ? 0 : lg - 1;
-  return f;
-}
-CARDIAC_D unsigned fastdiv(unsigned n, const FastDiv& f) { return f.d == 1 ? n : __umulhi(n, f.mul) >> f.shr; }
-
 template <class MD>
 struct RingArgs {
   StageArgs<MD> a;
   unsigned tiles_x, ntiles;   // ntiles < 2^31
   FastDiv per_member, per_row;
 };
-struct TilePos {
-  int x0, y0, bz;
-};
 template <class MD>
 CARDIAC_D TilePos tile_pos(const RingArgs<MD>& ra, unsigned t) {
-  const unsigned bz = fastdiv(t, ra.per_member), rem = t - bz * ra.per_member.d;
-  const unsigned ty = fastdiv(rem, ra.per_row), tx = rem - ty * ra.tiles_x;
-  return {(int)tx * TW, (int)ty * TH, (int)bz};
+  return tile_pos_of(t, ra.per_member, ra.per_row, ra.tiles_x, TW, TH);
 }
 
-// ------------------------------------------------------------------ PTX wrappers
-CARDIAC_D unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-CARDIAC_D void mbar_init(uint64_t* b, unsigned count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
-}
-CARDIAC_D void mbar_arrive(uint64_t* b) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
-}
-CARDIAC_D void mbar_arrive_expect_tx(uint64_t* b, unsigned bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes)
-               : "memory");
-}
-CARDIAC_D void mbar_wait(uint64_t* b, unsigned parity) {
-  unsigned ok;
-  do {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(ok)
-        : "r"(smem_u32(b)), "r"(parity)
-        : "memory");
-  } while (!ok);
-}
-CARDIAC_D void tma_load_4d(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, int c3,
-                           uint64_t* bar) {
-  asm volatile(
-      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes "
-      "[%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(smem_u32(dst)),
-      "l"(reinterpret_cast<uint64_t>(tm)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar))
-      : "memory");
-}
 CARDIAC_D void consumer_sync() { __syncthreads(); }
 
 template <class MD, int STENCIL, int KIND>
@@ -276,63 +222,6 @@ __global__ void __launch_bounds__(NTHREADS)
   }
 }
 
-// ------------------------------------------------------------------ host: tensor maps
-using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
-                                   CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
-                                   CUtensorMapFloatOOBfill);
-
-EncodeTiledFn encoder() {
-  static EncodeTiledFn fn = [] {
-    void* p = nullptr;
-    cudaDriverEntryPointQueryResult q;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
-        q != cudaDriverEntryPointSuccess)
-      p = nullptr;
-    return reinterpret_cast<EncodeTiledFn>(p);
-  }();
-  return fn;
-}
-
-struct MapKey {
-  const void* base;
-  int nx, ny, nf, batch, pitch, bw, bh;
-  long long fstride, bstride;
-  bool operator==(const MapKey& o) const { return std::memcmp(this, &o, sizeof(MapKey)) == 0; }
-};
-struct MapEntry {
-  MapKey key;
-  CUtensorMap map;
-};
-
-// 4-D view (x, y, field, batch member) of `nf` fields starting at `base`; box = bw x bh x nf x 1
-cudaError_t tensor_map(const double* base, const Problem& pb, int nf, int bw, int bh, CUtensorMap* out) {
-  static std::mutex mu;
-  static std::vector<MapEntry> cache;
-  MapKey k;
-  std::memset(&k, 0, sizeof(k));
-  k.base = base; k.nx = pb.nx; k.ny = pb.ny; k.nf = nf; k.batch = pb.batch; k.pitch = pb.pitch;
-  k.bw = bw; k.bh = bh; k.fstride = pb.fstride; k.bstride = pb.bstride;
-  std::lock_guard<std::mutex> lock(mu);
-  for (const MapEntry& e : cache)
-    if (e.key == k) { *out = e.map; return cudaSuccess; }
-  EncodeTiledFn enc = encoder();
-  if (!enc) return cudaErrorNotSupported;
-  const cuuint64_t gdim[4] = {(cuuint64_t)pb.nx, (cuuint64_t)pb.ny, (cuuint64_t)nf, (cuuint64_t)pb.batch};
-  const cuuint64_t gstr[3] = {(cuuint64_t)pb.pitch * 8, (cuuint64_t)pb.fstride * 8, (cuuint64_t)pb.bstride * 8};
-  const cuuint32_t box[4] = {(cuuint32_t)bw, (cuuint32_t)bh, (cuuint32_t)nf, 1};
-  const cuuint32_t estr[4] = {1, 1, 1, 1};
-  CUtensorMap m;
-  CUresult r = enc(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double*>(base), gdim, gstr, box, estr,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                   CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
-  if (cache.size() >= 256) cache.clear();
-  cache.push_back({k, m});
-  *out = m;
-  return cudaSuccess;
-}
-
 template <class MD, int STENCIL, int KIND>
 cudaError_t run_ring(const Problem& pb, const StageLaunch& st, cudaStream_t stream) {
   using L = SlotLayout<MD, STENCIL, KIND>;
@@ -376,16 +265,16 @@ cudaError_t run_ring(const Problem& pb, const StageLaunch& st, cudaStream_t stre
   ra.per_row = make_fastdiv((unsigned)tiles_x);
 
   CUtensorMap tm_halo, tm_gate, tm_y, tm_A, tm_B;
-  if ((e = tensor_map(a.in, pb, MD::ND, HP, L::HR, &tm_halo)) != cudaSuccess) return e;
+  if ((e = tensor_map_4d(a.in, pb, MD::ND, HP, L::HR, &tm_halo)) != cudaSuccess) return e;
   tm_gate = tm_halo;
   if (L::NG > 0 &&
-      (e = tensor_map(a.in + MD::ND * pb.fstride, pb, L::NG, TW, TH, &tm_gate)) != cudaSuccess)
+      (e = tensor_map_4d(a.in + MD::ND * pb.fstride, pb, L::NG, TW, TH, &tm_gate)) != cudaSuccess)
     return e;
   tm_y = tm_A = tm_B = tm_halo;
-  if (KIND != K_SELF && (e = tensor_map(a.y, pb, MD::NV, TW, TH, &tm_y)) != cudaSuccess) return e;
+  if (KIND != K_SELF && (e = tensor_map_4d(a.y, pb, MD::NV, TW, TH, &tm_y)) != cudaSuccess) return e;
   if (KIND == K_RK4F) {
-    if ((e = tensor_map(a.A, pb, MD::NV, TW, TH, &tm_A)) != cudaSuccess) return e;
-    if ((e = tensor_map(a.B, pb, MD::NV, TW, TH, &tm_B)) != cudaSuccess) return e;
+    if ((e = tensor_map_4d(a.A, pb, MD::NV, TW, TH, &tm_A)) != cudaSuccess) return e;
+    if ((e = tensor_map_4d(a.B, pb, MD::NV, TW, TH, &tm_B)) != cudaSuccess) return e;
   }
   long long grid = grid_of[dev].load(std::memory_order_relaxed);
   if (grid > ra.ntiles) grid = ra.ntiles;
@@ -415,12 +304,80 @@ cudaError_t ring_by_stencil(const Problem& pb, const StageLaunch& st, cudaStream
 
 }  // namespace
 
+// ------------------------------------------------------------------ host: tensor maps (declared in tma.cuh)
+namespace {
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
+                                   CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                   CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encoder() {
+  static EncodeTiledFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      p = nullptr;
+    return reinterpret_cast<EncodeTiledFn>(p);
+  }();
+  return fn;
+}
+
+struct MapKey {
+  const void* base;
+  int nx, ny, nf, batch, pitch, bw, bh;
+  long long fstride, bstride;
+  bool operator==(const MapKey& o) const { return std::memcmp(this, &o, sizeof(MapKey)) == 0; }
+};
+struct MapEntry {
+  MapKey key;
+  CUtensorMap map;
+};
+
+}  // namespace
+
+// 4-D view (x, y, field, batch member) of `nf` fields starting at `base`; box = bw x bh x nf x 1
+cudaError_t tensor_map_4d(const double* base, const Problem& pb, int nf, int bw, int bh, CUtensorMap* out) {
+  static std::mutex mu;
+  static std::vector<MapEntry> cache;
+  MapKey k;
+  std::memset(&k, 0, sizeof(k));
+  k.base = base; k.nx = pb.nx; k.ny = pb.ny; k.nf = nf; k.batch = pb.batch; k.pitch = pb.pitch;
+  k.bw = bw; k.bh = bh; k.fstride = pb.fstride; k.bstride = pb.bstride;
+  std::lock_guard<std::mutex> lock(mu);
+  for (const MapEntry& e : cache)
+    if (e.key == k) { *out = e.map; return cudaSuccess; }
+  EncodeTiledFn enc = encoder();
+  if (!enc) return cudaErrorNotSupported;
+  const cuuint64_t gdim[4] = {(cuuint64_t)pb.nx, (cuuint64_t)pb.ny, (cuuint64_t)nf, (cuuint64_t)pb.batch};
+  const cuuint64_t gstr[3] = {(cuuint64_t)pb.pitch * 8, (cuuint64_t)pb.fstride * 8, (cuuint64_t)pb.bstride * 8};
+  const cuuint32_t box[4] = {(cuuint32_t)bw, (cuuint32_t)bh, (cuuint32_t)nf, 1};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  CUtensorMap m;
+  CUresult r = enc(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double*>(base), gdim, gstr, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                   CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+  if (cache.size() >= 256) cache.clear();
+  cache.push_back({k, m});
+  *out = m;
+  return cudaSuccess;
+}
+
+bool tma_available() { return encoder() != nullptr; }
+
 bool stage_ring_supported(const Problem& pb, int kind) {
   if (kind != K_SELF && kind != K_BASE && kind != K_RK4F) return false;
   if (pb.nz > 1) return false;   // the ring tiles are 2-D
   // tensor-map limits: strides are multiples of 16 bytes by construction (pitch % 16 == 0)
   const long long ntiles = (long long)((pb.nx + TW - 1) / TW) * ((pb.ny + TH - 1) / TH) * pb.batch;
-  return ntiles < (1LL << 31) && encoder() != nullptr;
+  return ntiles < (1LL << 31) && tma_available();
+}
+
+bool pair_tma_supported(const Problem& pb) {
+  if (pb.nz > 1 || pb.integrator > I_RK4) return false;
+  const long long ntiles = (long long)((pb.nx + 63) / 64) * ((pb.ny + 23) / 24) * pb.batch;
+  return ntiles < (1LL << 31) && tma_available();
 }
 
 cudaError_t launch_stage_ring(const Problem& pb, const StageLaunch& st, cudaStream_t stream) {

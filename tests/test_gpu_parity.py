@@ -64,9 +64,10 @@ CASES += [(BOCF, s, i) for s in (LAP5, LAP9X4, BOX9) for i in (RL, IE)]
 # CARDIAC_PLAN_* (+ parameter): STAGE with its DIRECT kernels, STAGE with the TMA-ring kernels
 # (forced: AUTO would pick DIRECT at these oracle-sized grids), FUSED
 # PAIR (two substeps per launch)
-STAGE, RING, FUSED, PERSISTENT, PAIR = (1, 1), (1, 2), 2, 3, 4
+# PAIR (two substeps per launch) with its DIRECT kernels and with the TMA-fed persistent kernels
+STAGE, RING, FUSED, PERSISTENT, PAIR, PAIRT = (1, 1), (1, 2), 2, 3, (4, 1), (4, 2)
 PLAN_CASES = [(m, s, i, STAGE) for (m, s, i) in CASES]
-PLAN_CASES += [(m, s, i, p) for (m, s, i) in CASES if i in (EULER, HEUN, RK4) for p in (RING, FUSED, PAIR)]
+PLAN_CASES += [(m, s, i, p) for (m, s, i) in CASES if i in (EULER, HEUN, RK4) for p in (RING, FUSED, PAIR, PAIRT)]
 
 
 @pytest.mark.parametrize("model,stencil,integ,plan", PLAN_CASES)
@@ -210,7 +211,7 @@ def test_persistent_plan_limits_and_auto(C):
 
 @pytest.mark.parametrize("model,stencil,integ", [(FHN, LAP9X4, RK4), (KARMA, LAP5, RK4), (BOCF, LAP9X4, RK4),
                                                  (FHN, LAP5, EULER), (BOCF, BOX9, HEUN)])
-@pytest.mark.parametrize("plan", [STAGE, RING, FUSED, PAIR])
+@pytest.mark.parametrize("plan", [STAGE, RING, FUSED, PAIR, PAIRT])
 def test_parity_periodic_boundary(C, model, stencil, integ, plan):
     cfg, Z = make(model, 37, 50, stencil, integ, boundary=1)
     got = gpu_run(C, cfg, Z, 30, plan=plan)
@@ -219,7 +220,7 @@ def test_parity_periodic_boundary(C, model, stencil, integ, plan):
 
 
 @pytest.mark.parametrize("model", [KARMA, BOCF])
-@pytest.mark.parametrize("plan", [STAGE, RING, FUSED, PAIR])
+@pytest.mark.parametrize("plan", [STAGE, RING, FUSED, PAIR, PAIRT])
 def test_parity_tanhfree_variant(C, model, plan):
     cfg, Z = make(model, 40, 33, LAP9X4, RK4, variant=1)
     got = gpu_run(C, cfg, Z, 50, plan=plan)
@@ -231,7 +232,7 @@ def test_parity_tanhfree_variant(C, model, plan):
 
 @pytest.mark.parametrize("model,stencil,nx,ny", [(FHN, LAP5, 3, 3), (FHN, LAP9X4, 5, 5), (KARMA, LAP9X4, 5, 64),
                                                  (BOCF, LAP5, 200, 3), (FHN, BOX9, 3, 17), (KARMA, LAP5, 33, 4)])
-@pytest.mark.parametrize("plan", [STAGE, RING, FUSED, PAIR])
+@pytest.mark.parametrize("plan", [STAGE, RING, FUSED, PAIR, PAIRT])
 def test_parity_degenerate_sizes(C, model, stencil, nx, ny, plan):
     """Minimum sizes 2r+1 (every stencil arm reflects; the fused window folds the grid several
     times over) and thin strips."""
@@ -241,7 +242,7 @@ def test_parity_degenerate_sizes(C, model, stencil, nx, ny, plan):
     assert maxabs(got, ref) <= tol(20)
 
 
-@pytest.mark.parametrize("plan", [STAGE, RING, FUSED, PAIR])
+@pytest.mark.parametrize("plan", [STAGE, RING, FUSED, PAIR, PAIRT])
 def test_batch_members_independent_of_position(C, plan):
     cfg, Z = make(KARMA, 48, 40, LAP5, RK4, batch=5, seed=3)
     def gpu_run_p(C, cfg, Z, n):
@@ -261,7 +262,8 @@ def test_batch_members_independent_of_position(C, plan):
                                               (FHN, EULER, RING), (BOCF, RK4, RING), (KARMA, HEUN, RING),
                                               (BOCF, RL, STAGE), (FHN, EULER, FUSED), (FHN, RK4, FUSED),
                                               (KARMA, HEUN, FUSED), (BOCF, EULER, FUSED),
-                                              (BOCF, RK4, PAIR), (FHN, EULER, PAIR), (KARMA, HEUN, PAIR)])
+                                              (BOCF, RK4, PAIR), (FHN, EULER, PAIR), (KARMA, HEUN, PAIR),
+                                              (BOCF, RK4, PAIRT), (FHN, EULER, PAIRT), (KARMA, HEUN, PAIRT)])
 def test_step_composition_and_determinism_bitwise(C, model, integ, plan):
     """step(a); step(b) == step(a+b), graph replay == direct launches, temporally blocked Euler ==
     single Euler steps, run-to-run identical."""
@@ -290,13 +292,14 @@ def test_fused_many_tiles_matches_stage_plan_and_oracle(C):
 @pytest.mark.parametrize("model,stencil,integ,bc", [(BOCF, LAP9X4, RK4, 0), (BOCF, LAP5, RK4, 1), (BOCF, BOX9, HEUN, 0),
                                                     (BOCF, LAP9X4, EULER, 1), (FHN, LAP9X4, RK4, 0), (KARMA, BOX9, RK4, 1),
                                                     (KARMA, LAP5, HEUN, 0), (FHN, LAP5, EULER, 0)])
-def test_pair_plan_many_tiles_bitwise_equal_to_stage_plan(C, model, stencil, integ, bc):
+@pytest.mark.parametrize("impl", [PAIR, PAIRT])
+def test_pair_plan_many_tiles_bitwise_equal_to_stage_plan(C, model, stencil, integ, bc, impl):
     """4 x 8 tiles of 64 x 24 cells with ragged edges (odd width), interior tiles (branch-free, 128-bit
     path) and rim tiles (ghost cells evaluated at their images): the ring cells a tile recomputes for
     its neighbours, and the combinations of the two fused substeps, are the stage plan's arithmetic —
     the same bits; an odd number of Euler steps ends with one stage launch."""
     cfg, Z = make(model, 251, 170, stencil, integ, seed=21, boundary=bc, batch=2)
-    got = gpu_run(C, cfg, Z, 13, plan=PAIR)
+    got = gpu_run(C, cfg, Z, 13, plan=impl)
     ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 13)
     assert maxabs(got, ref) <= tol(13)
     assert np.array_equal(got, gpu_run(C, cfg, Z, 13, plan=STAGE))
@@ -305,12 +308,13 @@ def test_pair_plan_many_tiles_bitwise_equal_to_stage_plan(C, model, stencil, int
 @pytest.mark.parametrize("nx,ny", [(64, 24), (65, 25), (66, 26), (67, 23), (68, 48), (69, 47), (128, 49), (130, 72),
                                    (63, 22), (5, 100), (200, 5), (132, 28)])
 @pytest.mark.parametrize("stencil,bc", [(LAP9X4, 0), (LAP9X4, 1), (BOX9, 0), (LAP5, 1)])
-def test_pair_plan_tile_edges(C, nx, ny, stencil, bc):
+@pytest.mark.parametrize("impl", [PAIR, PAIRT])
+def test_pair_plan_tile_edges(C, nx, ny, stencil, bc, impl):
     """Grid sizes around the 64 x 24 tile and its 4-cell / r-row margins: exactly one tile, one cell or one
     pair more, ghost cells inside a ragged tile, tiles whose ring is entirely ghost cells, strips thinner
     than a ring.  Bitwise the stage plan, and the oracle."""
     cfg, Z = make(BOCF, nx, ny, stencil, RK4, seed=nx * 131 + ny, boundary=bc)
-    got = gpu_run(C, cfg, Z, 3, plan=PAIR)
+    got = gpu_run(C, cfg, Z, 3, plan=impl)
     assert np.array_equal(got, gpu_run(C, cfg, Z, 3, plan=STAGE))
     assert maxabs(got, O.step(BOCF, Z, cfg.dx, cfg.dt, cfg.scheme, 3)) <= tol(3)
 
@@ -319,13 +323,13 @@ def test_pair_plan_limits(C):
     cfg, _ = make(BOCF, 40, 40, LAP5, RL)
     with C.Context.from_config(cfg) as ctx:
         with pytest.raises(C.CardiacError):
-            C.cardiac_set_plan(ctx.ctx, PAIR, 0)              # gate integrators: plan STAGE only
+            C.cardiac_set_plan(ctx.ctx, PAIR[0], 0)           # gate integrators: plan STAGE only
     cfg, _ = make(BOCF, 40, 40, LAP5, RK4)
     with C.Context.from_config(cfg) as ctx:
         with pytest.raises(C.CardiacError):
-            C.cardiac_set_plan(ctx.ctx, PAIR, 3)
+            C.cardiac_set_plan(ctx.ctx, PAIR[0], 3)
     # AUTO: the 4-field model with RK4 from 1536^2 cells (config 4 included), Heun from 12 Mi; STAGE below
-    for n, integ, want in [(2048, RK4, PAIR), (1536, RK4, PAIR), (1280, RK4, 1), (2048, HEUN, 1), (3584, HEUN, PAIR), (2048, EULER, 1)]:
+    for n, integ, want in [(2048, RK4, PAIR[0]), (1536, RK4, PAIR[0]), (1280, RK4, 1), (2048, HEUN, 1), (3584, HEUN, PAIR[0]), (2048, EULER, 1)]:
         ctx = C.cardiac_create(BOCF, n, n, 0.03, 0.09, LAP9X4 | integ_bits(C, integ), 1)
         try:
             assert C.cardiac_get_plan(ctx) == want, (n, integ)
@@ -351,11 +355,11 @@ def test_plan_switch_keeps_state(C):
         ctx.step(4)
         C.cardiac_set_plan(ctx.ctx, FUSED, 0)
         ctx.step(2)
-        C.cardiac_set_plan(ctx.ctx, PAIR, 0)          # rotates the state through three buffers
+        C.cardiac_set_plan(ctx.ctx, *PAIR)            # rotates the state through three buffers
         ctx.step(2)
         C.cardiac_set_plan(ctx.ctx, FUSED, 0)
         ctx.step(1)
-        C.cardiac_set_plan(ctx.ctx, PAIR, 0)
+        C.cardiac_set_plan(ctx.ctx, *PAIRT)
         ctx.step(2)
         C.cardiac_set_plan(ctx.ctx, *STAGE)
         ctx.step(1)
@@ -477,7 +481,7 @@ def test_configs_full_size_step1_and_step100(C, idx, omp):
     Z = W.initial_state(cfg)
     with C.Context.from_config(cfg) as ctx:
         if idx == 4:
-            assert ctx.plan == PAIR
+            assert ctx.plan == PAIR[0]
         ctx.set_state(Z)
         ctx.step(1)
         got1 = ctx.get_state()

@@ -6,15 +6,21 @@
 // instructions PLUS ~2x as many integer/move instructions (64-bit polynomial coefficients are
 // materialised with two 32-bit moves each, the division carries a slow-path call).  ncu on the v1
 // kernel showed BOCF issue-bound at 647 warp-instructions per cell-stage of which only 222 were
-// FP64 (profiles/r1_v1_cfg4_stage_full.csv).  The versions here keep every coefficient in the
-// constant bank (a DFMA operand, no move) and have no branches:
-//   rcp_pos : MUFU.RCP64H seed (rcp.approx.ftz.f64, rel. error 2^-23) + two Newton steps -> <= 1 ulp
-//   exp_c   : x clamped to [-700, 700], n = rint(x log2 e) by the 1.5*2^52 trick, two-term
-//             Cody-Waite reduction, degree-13 Taylor polynomial on |r| <= ln2/2 (remainder 4e-18),
-//             2^n added into the exponent field -> <= 1 ulp (+ the clamp: exact 0/1 limits of the
-//             logistic are reached to 1e-304)
-// Neither is correctly rounded; DESIGN.md "Tolerance" budgets 1 ulp per operation against the
-// oracle's glibc tanh/exp and IEEE division.
+// FP64 (profiles/r1_v1_cfg4_stage_full.csv).  Measured in round 2: an FP64
+// instruction holds a scheduler's issue port for ~2.2 cycles and nothing else issues meanwhile, so
+// what a BOCF substep costs is 2.2 x (FP64 instructions) + (all others), and three exponentials and five
+// reciprocals were half of its 138 FP64 instructions.  The versions here have no branches and spend
+// as few instructions as 1-2 ulp allow:
+//   rcp_pos : MUFU.RCP64H seed (rcp.approx.ftz.f64, rel. error e0 <= 2^-23) + ONE third-order step
+//             r (1 + e + e^2), e = 1 - b r (remainder e^3 = 2^-69): 3 DFMA                    -> <= 1 ulp
+//   exp_c   : x clamped to [-700, 700], n = rint(x 128/ln2) by the 1.5*2^52 trick, two-term Cody-Waite
+//             reduction r = x - n ln2/128 (|r| <= 0.0027), e^x = 2^(n>>7) T[n&127] (1 + q),
+//             T[j] = 2^(j/128) from a 1 KB table read through L1 (exp_table.inc; a constant-bank table
+//             would serialise on the 32 different indices of a warp), q = e^r - 1 = r P4(r) (degree-4
+//             Taylor, remainder r^6/720 = 5e-19), result fma(T, q, T): 10 FP64 instructions (the
+//             degree-13 polynomial of round 1: 17)                                           -> <= 1.5 ulp
+// Neither is correctly rounded; DESIGN.md "Tolerance" budgets 1-2 ulp per operation against the
+// oracle's glibc tanh/exp and IEEE division (checked value by value, tests/test_gpu_math.py).
 #pragma once
 
 namespace cardiac {
@@ -23,11 +29,10 @@ namespace cardiac {
 #define CARDIAC_D __device__ __forceinline__
 #endif
 
-// 1/k!, k = 13 .. 2 (Horner order), then ln2 split and log2(e)
-__constant__ double kExpC[12] = {
-    1.0 / 6227020800.0, 1.0 / 479001600.0, 1.0 / 39916800.0, 1.0 / 3628800.0,
-    1.0 / 362880.0,     1.0 / 40320.0,     1.0 / 5040.0,     1.0 / 720.0,
-    1.0 / 120.0,        1.0 / 24.0,        1.0 / 6.0,        0.5};
+// 2^(j/128), j = 0 .. 127 (global memory, read through L1 with ld.global.nc)
+__device__ const double kExp2Tab[128] = {
+#include "exp_table.inc"
+};
 
 // clamp(t, 0, 1) and clamp(x, -700, 700) decided on the HIGH WORD with integer instructions.
 // fmin/fmax on doubles have no single sm_100a instruction: each expands to DSETP (on the FP64 pipe)
@@ -53,29 +58,30 @@ CARDIAC_D double clamp700(double x) {
 CARDIAC_D double rcp_pos(double b) {
   double r;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(b));
-  double e = fma(-b, r, 1.0);
-  r = fma(r, e, r);
-  e = fma(-b, r, 1.0);
-  return fma(r, e, r);
+  const double e = fma(-b, r, 1.0);
+  return fma(r, fma(e, e, e), r);
 }
 
+// (literals on purpose: with the coefficients in a __constant__ array ptxas loads them with LDC instead of
+// folding them into the DFMAs, measured 2 % slower on the BOCF pair kernels)
 CARDIAC_D double exp_c(double x) {
-  const double kL2E = 1.4426950408889634074;      // log2(e)
-  const double kLn2Hi = 0.6931471787393093;       // ln2 with the low 24 mantissa bits zero: n*hi exact
-  const double kLn2Lo = 1.8206359985041462e-09;   // ln2 - kLn2Hi (60-digit ln2)
+  const double k128L2E = 184.6649652337873;       // 128 log2(e)
+  const double kLn2Hi = 0.6931471787393093 / 128.0;       // ln2/128, low 24 mantissa bits zero: n*hi exact
+  const double kLn2Lo = 1.8206359985041462e-09 / 128.0;   // ln2/128 - hi (60-digit ln2)
   const double kMagic = 6755399441055744.0;       // 1.5 * 2^52: fma(x, c, magic) rounds x c to an integer
   x = clamp700(x);
-  double t = fma(x, kL2E, kMagic);
-  int n = __double2loint(t);
-  double fn = t - kMagic;
+  const double t = fma(x, k128L2E, kMagic);
+  const int n = __double2loint(t);                // |n| <= 129271
+  const double fn = t - kMagic;
   double r = fma(fn, -kLn2Hi, x);
   r = fma(fn, -kLn2Lo, r);
-  double p = kExpC[0];
-#pragma unroll
-  for (int i = 1; i < 12; ++i) p = fma(p, r, kExpC[i]);
+  const double T = __ldg(&kExp2Tab[n & 127]);
+  double p = fma(1.0 / 120.0, r, 1.0 / 24.0);     // (e^r - 1)/r = 1 + r/2 + r^2/6 + r^3/24 + r^4/120 (+ r^5/720)
+  p = fma(p, r, 1.0 / 6.0);
+  p = fma(p, r, 0.5);
   p = fma(p, r, 1.0);
-  p = fma(p, r, 1.0);   // p = e^r in [0.70, 1.42]
-  return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));  // p * 2^n, |n| <= 1010
+  const double v = fma(T, p * r, T);              // T e^r in [1, 2.01)
+  return __hiloint2double(__double2hiint(v) + ((n >> 7) << 20), __double2loint(v));  // v * 2^(n>>7), |n>>7| <= 1010
 }
 
 }  // namespace cardiac

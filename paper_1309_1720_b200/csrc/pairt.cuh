@@ -57,18 +57,18 @@ struct PairTArgs {
   FastDiv per_member, per_row;
 };
 
-constexpr int kPairTThreads = 384;
-template <class MD>
-CARDIAC_D TilePos tile_pos(const PairTArgs<MD>& a, unsigned t) {
-  return tile_pos_of(t, a.per_member, a.per_row, a.tiles_x, 64, 24);
-}
+// tile height and threads per CTA (a warp = TH / (NT / 32) tile rows)
+template <int TH_, int NT_>
+struct PairTGeom {
+  static constexpr int TH = TH_, NT = NT_;
+};
 
-template <class MD, int STENCIL, int KA, int KB>
+template <class MD, int STENCIL, int KA, int KB, class PG>
 struct PairTShape {
   static constexpr int NV = MD::NV, ND = MD::ND, NG = NV - ND;
   static constexpr int R = stencil_radius(STENCIL);
   static constexpr int HX = 2;                         // x margin of the window: r rounded up to a pair
-  static constexpr int TW = 64, TH = 24, NT = kPairTThreads, NW = NT / 32;
+  static constexpr int TW = 64, TH = PG::TH, NT = PG::NT, NW = NT / 32;
   static constexpr int PW = TW / 2;                    // pairs per tile row = lanes
   static constexpr int WW = TW + 2 * HX, WPW = WW / 2, WH = TH + 2 * R, WSZ = WW * WH, TSZ = TW * TH;
   static constexpr int BW = TW + 4 * HX, BH = TH + 4 * R, BSZ = BW * BH;   // input box of a diffusing field
@@ -121,10 +121,10 @@ CARDIAC_D void patch_box(double* __restrict__ box, int nf, int bw, int bh, int b
 // Substep KA of the pair at window position (wpx, wy), every operand from the P1 slot, no boundary logic.
 // FULL: all fields (tile cells); otherwise the diffusing fields only (ring cells: the rest of the reaction
 // is dead code).  Same instruction sequence per cell as pair_from_global (pair.cuh) / the stage kernels.
-template <class MD, int STENCIL, int KA, int KB, bool FULL>
+template <class MD, int STENCIL, int KA, int KB, class PG, bool FULL>
 CARDIAC_D void pairt_substep_a(const PairTArgs<MD>& a, const unsigned char* __restrict__ slot, int wpx, int wy,
                                double2 (&res)[MD::NV]) {
-  using S = PairTShape<MD, STENCIL, KA, KB>;
+  using S = PairTShape<MD, STENCIL, KA, KB, PG>;
   constexpr int NV = S::NV, ND = S::ND, NQ = FULL ? NV : ND, R = S::R, HX = S::HX;
   const double* inu = reinterpret_cast<const double*>(slot + S::OFF_INU);
   const double* ing = reinterpret_cast<const double*>(slot + S::OFF_ING);
@@ -160,12 +160,12 @@ CARDIAC_D void pairt_substep_a(const PairTArgs<MD>& a, const unsigned char* __re
   }
 }
 
-template <class MD, int STENCIL, int KA, int KB, bool WRITE_P>
-__global__ void __launch_bounds__(kPairTThreads, 1)
+template <class MD, int STENCIL, int KA, int KB, bool WRITE_P, class PG>
+__global__ void __launch_bounds__(PG::NT, 1)
     pair_tma_kernel(const __grid_constant__ PairTArgs<MD> a, const __grid_constant__ CUtensorMap tm_inu,
                     const __grid_constant__ CUtensorMap tm_ing, const __grid_constant__ CUtensorMap tm_yu,
                     const __grid_constant__ CUtensorMap tm_yg, const __grid_constant__ CUtensorMap tm_p) {
-  using S = PairTShape<MD, STENCIL, KA, KB>;
+  using S = PairTShape<MD, STENCIL, KA, KB, PG>;
   constexpr int NV = S::NV, ND = S::ND, NG = S::NG, R = S::R, HX = S::HX, TW = S::TW, TH = S::TH, PW = S::PW;
   constexpr int WW = S::WW, WPW = S::WPW, WH = S::WH, WSZ = S::WSZ, TSZ = S::TSZ, NT = S::NT, NW = S::NW;
   constexpr int NSLOT1 = S::NSLOT1;
@@ -181,7 +181,7 @@ __global__ void __launch_bounds__(kPairTThreads, 1)
 
   // the box copies of tile t (one elected thread)
   auto issue1 = [&](unsigned t, int s) {
-    const TilePos tp = tile_pos(a, t);
+    const TilePos tp = tile_pos_of(t, a.per_member, a.per_row, a.tiles_x, TW, TH);
     unsigned char* slot = pt_smem + s * S::P1_BYTES;
     mbar_arrive_expect_tx(full1 + s, S::TX1);
     tma_load_4d(slot + S::OFF_INU, &tm_inu, tp.x0 - 2 * HX, tp.y0 - 2 * R, 0, tp.bz, full1 + s);
@@ -192,7 +192,7 @@ __global__ void __launch_bounds__(kPairTThreads, 1)
     }
   };
   auto issue2 = [&](unsigned t) {
-    const TilePos tp = tile_pos(a, t);
+    const TilePos tp = tile_pos_of(t, a.per_member, a.per_row, a.tiles_x, TW, TH);
     mbar_arrive_expect_tx(full2, S::TX2);
     tma_load_4d(p2, &tm_p, tp.x0, tp.y0, 0, tp.bz, full2);
   };
@@ -219,7 +219,7 @@ __global__ void __launch_bounds__(kPairTThreads, 1)
   int s1 = 0;
   unsigned ph1 = 0, ph2 = 0;
   for (unsigned t = blockIdx.x; t < a.ntiles; t += gridDim.x) {
-    const TilePos tp = tile_pos(a, t);
+    const TilePos tp = tile_pos_of(t, a.per_member, a.per_row, a.tiles_x, TW, TH);
     const int x0 = tp.x0, y0 = tp.y0;
     const long long base = (long long)tp.bz * a.g.bstride;
     unsigned char* const slot = pt_smem + s1 * S::P1_BYTES;
@@ -243,7 +243,7 @@ __global__ void __launch_bounds__(kPairTThreads, 1)
     for (int py = warp; py < TH; py += NW) {   // tile cells: every field
       if (y0 + py > ny - 1 + R) break;          // beyond the ghost rows of a ragged tile
       double2 res[NV];
-      pairt_substep_a<MD, STENCIL, KA, KB, true>(a, slot, lane + HX / 2, py + R, res);
+      pairt_substep_a<MD, STENCIL, KA, KB, PG, true>(a, slot, lane + HX / 2, py + R, res);
 #pragma unroll
       for (int q = 0; q < NV; ++q) {
         if (q < ND) *reinterpret_cast<double2*>(sw + q * WSZ + (py + R) * WW + HX + 2 * lane) = res[q];
@@ -263,7 +263,7 @@ __global__ void __launch_bounds__(kPairTThreads, 1)
       }
       if (y0 - R + wy <= ny - 1 + R) {
         double2 res[NV];
-        pairt_substep_a<MD, STENCIL, KA, KB, false>(a, slot, wpx, wy, res);
+        pairt_substep_a<MD, STENCIL, KA, KB, PG, false>(a, slot, wpx, wy, res);
 #pragma unroll
         for (int q = 0; q < ND; ++q) *reinterpret_cast<double2*>(sw + q * WSZ + wy * WW + 2 * wpx) = res[q];
       }

@@ -7,10 +7,15 @@
 
 namespace cardiac {
 
-template <class MD, int STENCIL, int KA, int KB, bool WRITE_P>
+// 64 x 24 tiles on 12 warps (two rows per warp) — or, experimental, 64 x 16 on 16 warps (pb.pair_impl == 3)
+using PairTTile = PairTGeom<24, 384>;
+using PairTTile16 = PairTGeom<16, 512>;
+using PairTTile20 = PairTGeom<20, 640>;
+
+template <class MD, int STENCIL, int KA, int KB, bool WRITE_P, class PG = PairTTile>
 cudaError_t pairt_run(const Problem& pb, const PairTLaunch& pl, cudaStream_t stream) {
-  using S = PairTShape<MD, STENCIL, KA, KB>;
-  auto kern = pair_tma_kernel<MD, STENCIL, KA, KB, WRITE_P>;
+  using S = PairTShape<MD, STENCIL, KA, KB, PG>;
+  auto kern = pair_tma_kernel<MD, STENCIL, KA, KB, WRITE_P, PG>;
   // per instantiation and device: the shared-memory limit and the size of the persistent grid (one CTA per SM)
   static PerDeviceOnce configured;
   static std::atomic<int> sms_of[64];
@@ -76,13 +81,13 @@ cudaError_t pairt_run(const Problem& pb, const PairTLaunch& pl, cudaStream_t str
   return cudaLaunchKernelEx(&cfg, kern, a, tm_inu, tm_ing, tm_yu, tm_yg, tm_p);
 }
 
-template <class MD, int STENCIL>
+template <class MD, int STENCIL, class PG = PairTTile>
 cudaError_t pairt_by_kind(const Problem& pb, const PairTLaunch& pl, cudaStream_t s) {
   if (pl.ka == K_SELF && pl.kb == K_BASE)
-    return pl.out2 ? pairt_run<MD, STENCIL, K_SELF, K_BASE, true>(pb, pl, s)     // RK4 substeps 1+2 (+ P)
-                   : pairt_run<MD, STENCIL, K_SELF, K_BASE, false>(pb, pl, s);   // Heun
-  if (pl.ka == K_BASE && pl.kb == K_RK4F) return pairt_run<MD, STENCIL, K_BASE, K_RK4F, false>(pb, pl, s);   // RK4 substeps 3+4
-  if (pl.ka == K_SELF && pl.kb == K_SELF) return pairt_run<MD, STENCIL, K_SELF, K_SELF, false>(pb, pl, s);   // two Euler steps
+    return pl.out2 ? pairt_run<MD, STENCIL, K_SELF, K_BASE, true, PG>(pb, pl, s)     // RK4 substeps 1+2 (+ P)
+                   : pairt_run<MD, STENCIL, K_SELF, K_BASE, false, PG>(pb, pl, s);   // Heun
+  if (pl.ka == K_BASE && pl.kb == K_RK4F) return pairt_run<MD, STENCIL, K_BASE, K_RK4F, false, PG>(pb, pl, s);   // RK4 substeps 3+4
+  if (pl.ka == K_SELF && pl.kb == K_SELF) return pairt_run<MD, STENCIL, K_SELF, K_SELF, false, PG>(pb, pl, s);   // two Euler steps
   return cudaErrorInvalidValue;
 }
 
@@ -90,7 +95,12 @@ template <class MD>
 cudaError_t pairt_by_stencil(const Problem& pb, const PairTLaunch& pl, cudaStream_t s) {
   switch (pb.stencil) {
     case S_LAP5: return pairt_by_kind<MD, S_LAP5>(pb, pl, s);
-    case S_LAP9X4: return pairt_by_kind<MD, S_LAP9X4>(pb, pl, s);
+    case S_LAP9X4:
+      if constexpr (MD::NV == 4)
+        if (pb.pair_impl == 3) return pairt_by_kind<MD, S_LAP9X4, PairTTile16>(pb, pl, s);
+      if constexpr (MD::NV == 4)
+        if (pb.pair_impl == 4) return pairt_by_kind<MD, S_LAP9X4, PairTTile20>(pb, pl, s);
+      return pairt_by_kind<MD, S_LAP9X4>(pb, pl, s);
     case S_BOX9: return pairt_by_kind<MD, S_BOX9>(pb, pl, s);
   }
   return cudaErrorInvalidValue;

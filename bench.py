@@ -47,12 +47,13 @@ def algo_bytes_per_cell_step(cfg) -> int:
 # Algorithmic FP64 work per cell-step of the five configs: FP64 instructions (DFMA + DMUL + DADD) and
 # flops (DFMA = 2) of the non-redundant update of ONE cell through all substeps, counted in the SASS of
 # the stage kernels (cuobjdump, body of ring_stage_kernel<model, stencil, kind>, per pair / 2; DESIGN.md
-# "Roofline"; re-counted whenever models.cuh / fastmath.cuh change: profiles/README.md).
+# "Roofline"); written by `python -m paper_1309_1720_b200.sass_count`, re-run whenever models.cuh /
+# fastmath.cuh change (round 1, degree-13 exp and two-step reciprocal: Karma 220 / 342, BOCF 633 / 1045).
 FP64_PER_CELL_STEP = {   # (model, stencil, integrator): (instructions, flops)
     (W.FHN, W.LAP5, W.EULER): (18, 26),
     (W.FHN, W.LAP9X4, W.RK4): (120, 170),
-    (W.KARMA, W.LAP5, W.RK4): (220, 342),
-    (W.BOCF, W.LAP9X4, W.RK4): (633, 1045),
+    (W.KARMA, W.LAP5, W.RK4): (188, 274),
+    (W.BOCF, W.LAP9X4, W.RK4): (529.5, 825.5),
 }
 # nominal FP64 peak, for context only: 148 SM x 64 FP64 lanes/clk x 2 x 1.965 GHz (the measured one is
 # taken live by cardiac_measure_fp64_peak, include/cardiac_diag.h)

@@ -108,6 +108,7 @@ struct Model<M_BOCF, VARIANT> {
     double inv_tau_fi, tau_o1, dtau_o, tau_so1, dtau_so, k_so, u_so;
     double tau_s1, dtau_s, k_s, u_s, inv_tau_si, inv_tau_winf, winf_star;
     double m2k_wm, m2k_s, m2k_so;  // -2 k: exponent scale of 1 + e^{-2 k (u - u0)}
+    int same_o_vm;                 // theta_o == theta_v^- (the epicardial set): H_k(u - theta_o) is H_k(u - theta_v^-)
   };
   static void derive(const double* p, Params& q) {
     q.D[0] = p[0]; q.k = p[1]; q.u_o = p[2]; q.u_u = p[3]; q.th_v = p[4]; q.th_w = p[5];
@@ -120,12 +121,14 @@ struct Model<M_BOCF, VARIANT> {
     q.tau_s1 = p[23]; q.dtau_s = p[24] - p[23]; q.k_s = p[25]; q.u_s = p[26];
     q.inv_tau_si = 1.0 / p[27]; q.inv_tau_winf = 1.0 / p[28]; q.winf_star = p[29];
     q.m2k_wm = -2.0 * q.k_wm; q.m2k_s = -2.0 * q.k_s; q.m2k_so = -2.0 * q.k_so;
+    q.same_o_vm = q.th_o == q.th_vm;
   }
 
   // gate equations x' = alpha_x(u) x + beta_x(u), x = v, w, s (Q9)
   CARDIAC_D static void gates(const Params& q, double u, double (&alpha)[3], double (&beta)[3]) {
     double h_v = hk(u - q.th_v, q.k), h_w = hk(u - q.th_w, q.k);
-    double h_o = hk(u - q.th_o, q.k), h_vm = hk(u - q.th_vm, q.k);
+    // (uniform branch: with equal thresholds the two are the same instruction sequence on the same input)
+    double h_o = hk(u - q.th_o, q.k), h_vm = q.same_o_vm ? h_o : hk(u - q.th_vm, q.k);
     double inv_tau_vm = rcp_pos(fma(h_vm, q.dtau_vm, q.tau_v1m));
     double tau_s = fma(h_w, q.dtau_s, q.tau_s1);
     double inv_tau_wm, inv_tau_s, beta_s;

@@ -7,10 +7,11 @@
 
 namespace cardiac {
 
-// 64 x 24 tiles on 12 warps (two rows per warp) — or, experimental, 64 x 16 on 16 warps (pb.pair_impl == 3)
+// 64 x 24 tiles on 12 warps (two rows per warp, <= 168 registers).  Measured on B200, BOCF LAP9X4 RK4, us per
+// step at 2048^2 / 4096^2: 248 / 963; 64 x 16 on 16 warps (128 registers) 256 / 1001; 64 x 20 on 20 warps
+// (102 registers) 252 / 976 — more warps do not help: the schedulers' issue ports are what is busy
+// (DESIGN.md "FP64 issue"), and the smaller tiles recompute a larger ring.
 using PairTTile = PairTGeom<24, 384>;
-using PairTTile16 = PairTGeom<16, 512>;
-using PairTTile20 = PairTGeom<20, 640>;
 
 template <class MD, int STENCIL, int KA, int KB, bool WRITE_P, class PG = PairTTile>
 cudaError_t pairt_run(const Problem& pb, const PairTLaunch& pl, cudaStream_t stream) {
@@ -95,12 +96,7 @@ template <class MD>
 cudaError_t pairt_by_stencil(const Problem& pb, const PairTLaunch& pl, cudaStream_t s) {
   switch (pb.stencil) {
     case S_LAP5: return pairt_by_kind<MD, S_LAP5>(pb, pl, s);
-    case S_LAP9X4:
-      if constexpr (MD::NV == 4)
-        if (pb.pair_impl == 3) return pairt_by_kind<MD, S_LAP9X4, PairTTile16>(pb, pl, s);
-      if constexpr (MD::NV == 4)
-        if (pb.pair_impl == 4) return pairt_by_kind<MD, S_LAP9X4, PairTTile20>(pb, pl, s);
-      return pairt_by_kind<MD, S_LAP9X4>(pb, pl, s);
+    case S_LAP9X4: return pairt_by_kind<MD, S_LAP9X4>(pb, pl, s);
     case S_BOX9: return pairt_by_kind<MD, S_BOX9>(pb, pl, s);
   }
   return cudaErrorInvalidValue;

@@ -39,9 +39,11 @@ def test_exp_matches_libm_to_2ulp(C):
     got = probe(C, W.FHN, C.CARDIAC_PROBE_EXP, x)
     ref = np.exp(x)
     assert np.max(np.abs(got - ref) / ref) <= 2 * 2.3e-16
-    # clamped outside +-700: the logistic built on it still reaches its exact limits
+    # |x| limited to [700, 700.000123) beyond +-700 (high word clamped): finite, and the logistic built on it
+    # is at its 0 / 1 limit there
     out = probe(C, W.FHN, C.CARDIAC_PROBE_EXP, np.array([1e4, -1e4, 5e300, -5e300]))
-    assert np.allclose(out[[0, 2]], np.exp(700.0), rtol=1e-15) and np.allclose(out[[1, 3]], np.exp(-700.0), rtol=1e-15)
+    assert np.all(np.isfinite(out)) and np.all(out[[0, 2]] >= np.exp(700.0)) and np.all(out[[0, 2]] < np.exp(700.001))
+    assert np.all(out[[1, 3]] <= np.exp(-700.0)) and np.all(out[[1, 3]] > np.exp(-700.001))
 
 
 def test_reciprocal_to_1ulp(C):

@@ -328,8 +328,10 @@ def test_pair_plan_limits(C):
     with C.Context.from_config(cfg) as ctx:
         with pytest.raises(C.CardiacError):
             C.cardiac_set_plan(ctx.ctx, PAIR[0], 3)
-    # AUTO: the 4-field model with RK4 from 1536^2 cells (config 4 included), Heun from 12 Mi; STAGE below
-    for n, integ, want in [(2048, RK4, PAIR[0]), (1536, RK4, PAIR[0]), (1280, RK4, 1), (2048, HEUN, 1), (3584, HEUN, PAIR[0]), (2048, EULER, 1)]:
+    # AUTO: the 4-field model with RK4 from 4 x 148 tiles of 64 x 24 cells (1024^2; config 4 included), Heun from
+    # 12 Mi cells; STAGE below
+    for n, integ, want in [(2048, RK4, PAIR[0]), (1536, RK4, PAIR[0]), (1024, RK4, PAIR[0]), (768, RK4, 1), (2048, HEUN, 1),
+                           (3584, HEUN, PAIR[0]), (2048, EULER, 1)]:
         ctx = C.cardiac_create(BOCF, n, n, 0.03, 0.09, LAP9X4 | integ_bits(C, integ), 1)
         try:
             assert C.cardiac_get_plan(ctx) == want, (n, integ)

@@ -31,6 +31,7 @@ struct cardiac_ctx {
   cudaStream_t stream = nullptr;
   cudaStream_t cap_stream = nullptr;  // only ever used in capture mode
   int plan_req = CARDIAC_PLAN_AUTO, plan = CARDIAC_PLAN_STAGE, plan_param = 0;
+  int fused_impl = 0;   // plan FUSED: 0 = by size, 1 = one CTA per tile, 2 = persistent CTAs fed by TMA
   void* ws = nullptr;
   size_t ws_bytes = 0;
   bool ws_owned = false;
@@ -93,6 +94,11 @@ void carve(cardiac_ctx* c) {
 int fused_window_auto(const Problem& pb) {
   if (pb.nv > 2 || pb.integrator == I_EULER) return 1;
   const int H = pb.radius * stages_of(pb.integrator);
+  // Karma, RK4, halo 4: the 64 x 56 window on 896 threads, TMA-fed, from ~400 tiles (1024^2); measured above
+  if (pb.model == CARDIAC_KARMA && pb.integrator == I_RK4 && H <= 4 && fused_tma_supported(pb, 7, 1)) {
+    const long long n7 = (long long)((pb.nx + 55) / 56) * ((pb.ny + 47) / 48) * pb.batch;
+    if (n7 >= 400) return 7;
+  }
   auto ctas = [&](long long ew, long long eh) {
     const long long tw = ew - 2 * H, th = eh - 2 * H;
     return ((pb.nx + tw - 1) / tw) * ((pb.ny + th - 1) / th) * pb.batch;
@@ -147,8 +153,20 @@ int fused_window(const cardiac_ctx* c) {
 // Plan FUSED: one launch advances `ksteps` time steps (1, or kEulerBlock Euler steps), ping-pong.
 int enqueue_fused(cardiac_ctx* c, cudaStream_t s, int ksteps) {
   const int other = c->cur == 0 ? 1 : 0;   // (plan PAIR may have left the state in buffer 2)
-  TileLaunch tl{c->buf[c->cur], c->buf[other], ksteps, fused_window(c)};
-  cudaError_t e = launch_fused(c->pb, tl, s);
+  TileLaunch tl{c->buf[c->cur], c->buf[other], ksteps, c->fused_impl, fused_window(c)};
+  bool tma = false;
+  if (c->fused_impl != 1 && fused_tma_supported(c->pb, tl.window, ksteps)) {
+    if (c->fused_impl == 2) {
+      tma = true;
+    } else {   // AUTO: once every persistent CTA has several tiles to pipeline
+      const int ns = c->pb.integrator == I_RK4 ? 4 : (c->pb.integrator == I_HEUN ? 2 : ksteps);
+      int tw, th;
+      fused_tile_of(c->pb.integrator == I_EULER ? 1 : tl.window, c->pb.radius * ns, tw, th);
+      const long long ntiles = (long long)((c->pb.nx + tw - 1) / tw) * ((c->pb.ny + th - 1) / th) * c->pb.batch;
+      tma = tl.window == 7 ? ntiles >= 400 : ntiles >= kFusedTMinTiles * (tl.window == 2 ? 2 : 1);
+    }
+  }
+  cudaError_t e = tma ? launch_fusedt(c->pb, tl, s) : launch_fused(c->pb, tl, s);
   if (e != cudaSuccess) return fail_cuda(c, e, "fused launch");
   c->launches++;
   c->cur = other;
@@ -513,7 +531,8 @@ int cardiac_set_stream(cardiac_ctx* c, void* cuda_stream) {
 
 int cardiac_set_plan(cardiac_ctx* c, int plan, int param) {
   if (!c) return CARDIAC_ERR_INVALID;
-  int resolved = plan, rparam = 0;
+  int resolved = plan, rparam = 0, fimpl = 0;
+  if (param < 0) return fail(c, CARDIAC_ERR_INVALID, "plan parameter must be >= 0");
   const int integ = c->pb.integrator;
   const bool rk_like = integ == I_EULER || integ == I_HEUN || integ == I_RK4;
   if (plan == CARDIAC_PLAN_AUTO) resolved = auto_plan(c->pb);
@@ -526,15 +545,18 @@ int cardiac_set_plan(cardiac_ctx* c, int plan, int param) {
     return fail(c, CARDIAC_ERR_INVALID, "3-D contexts run plan STAGE only");
   } else if (resolved == CARDIAC_PLAN_FUSED) {
     if (!rk_like) return fail(c, CARDIAC_ERR_INVALID, "FUSED supports Euler, Heun and RK4 only");
+    fimpl = param >> 4;
+    param &= 15;
+    if (fimpl < 0 || fimpl > 2) return fail(c, CARDIAC_ERR_INVALID, "FUSED: implementation (parameter / 16) must be 0, 1 or 2");
     if (integ == I_EULER) {
       rparam = param == 0 ? kEulerBlock : param;
       if (rparam != 1 && rparam != kEulerBlock)
         return fail(c, CARDIAC_ERR_INVALID, "FUSED + Euler: steps per launch must be 1 or 4");
     } else {
-      if (param < 0 || param > 5 || (param >= 2 && c->pb.nv > 2) || (param >= 3 && integ != I_RK4))
+      if (param < 0 || param > 7 || param == 6 || (param >= 2 && c->pb.nv > 2) || (param >= 3 && integ != I_RK4))
         return fail(c, CARDIAC_ERR_INVALID,
                     "FUSED + Heun/RK4: parameter 0 (auto), 1 (80x48 window), 2 (48x40 window, 2-field models) "
-                    "or 3 / 4 / 5 (64x56 / 64x48 / 56x48 window, 2-field models, RK4)");
+                    "or 3 / 4 / 5 / 7 (64x56 / 64x48 / 56x48 / 64x56 on 896 threads, 2-field models, RK4)");
       rparam = param == 0 ? fused_window_auto(c->pb) : param;
     }
   } else if (resolved == CARDIAC_PLAN_PAIR) {
@@ -555,6 +577,9 @@ int cardiac_set_plan(cardiac_ctx* c, int plan, int param) {
   c->plan_req = plan;
   c->plan = resolved;
   c->plan_param = rparam;
+  if (fimpl == 2 && !fused_tma_supported(c->pb, integ == I_EULER ? 1 : rparam, integ == I_EULER ? rparam : 1))
+    return fail(c, CARDIAC_ERR_INVALID, "FUSED: the TMA implementation does not support this context / window");
+  c->fused_impl = fimpl;
   c->pb.stage_impl = resolved == CARDIAC_PLAN_STAGE ? rparam : 0;
   c->pb.pair_impl = resolved == CARDIAC_PLAN_PAIR ? rparam : 0;
   drop_graphs(c);

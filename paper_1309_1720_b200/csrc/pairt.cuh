@@ -92,19 +92,27 @@ struct PairTShape {
 };
 
 // Overwrite the ghost cells of a box — cells outside the grid, at most G beyond its edge — with the grid
-// cell the index reflects / wraps to, read from global memory (rim tiles only).  box: [nf][bh][bw], its cell
-// (0, 0) is grid cell (bx0, by0); src: field 0 of the same fields in global memory (batch member applied).
+// cell the index reflects / wraps to (rim tiles only).  box: [nf][bh][bw], its cell (0, 0) is grid cell
+// (bx0, by0); src: field 0 of the same fields in global memory (batch member applied).  No-flux: the image
+// of a ghost cell lies at most G inside the edge, i.e. inside the SAME box (every box reaches at least G
+// inside the grid on the side it sticks out of), so the patch is shared memory -> shared memory; images
+// are interior cells and ghost cells are never images, so no barrier is needed in between.  Periodic: the
+// image is on the other side of the grid and is read from global memory.
 template <int G>
 CARDIAC_D void patch_box(double* __restrict__ box, int nf, int bw, int bh, int bx0, int by0,
                          const double* __restrict__ src, const Geom& g, int tid, int nt) {
   const int nx = g.nx, ny = g.ny, bc = g.boundary;
+  auto image = [&](int q, int gx, int gy) -> double {   // (gx, gy) already reflected / wrapped into the grid
+    if (bc == B_NOFLUX) return box[(q * bh + (gy - by0)) * bw + (gx - bx0)];
+    return src[q * g.fstride + (long long)gy * g.pitch + gx];
+  };
   if (bx0 < 0 || bx0 + bw > nx) {   // ghost columns -G..-1 and nx..nx+G-1, every box row whose image exists
     for (int e = tid; e < nf * bh * 2 * G; e += nt) {
       const int q = e / (bh * 2 * G), rr = (e / (2 * G)) % bh, k = e % (2 * G);
       const int gx = k < G ? -1 - k : nx + (k - G), gy = by0 + rr;
       const int cc = gx - bx0;
       if (cc >= 0 && cc < bw && gy >= -G && gy < ny + G)
-        box[(q * bh + rr) * bw + cc] = src[q * g.fstride + (long long)bidx(gy, ny, bc) * g.pitch + bidx(gx, nx, bc)];
+        box[(q * bh + rr) * bw + cc] = image(q, bidx(gx, nx, bc), bidx(gy, ny, bc));
     }
   }
   if (by0 < 0 || by0 + bh > ny) {   // ghost rows -G..-1 and ny..ny+G-1 over the columns inside the grid
@@ -112,8 +120,7 @@ CARDIAC_D void patch_box(double* __restrict__ box, int nf, int bw, int bh, int b
       const int q = e / (2 * G * bw), k = (e / bw) % (2 * G), cc = e % bw;
       const int gy = k < G ? -1 - k : ny + (k - G), gx = bx0 + cc;
       const int rr = gy - by0;
-      if (rr >= 0 && rr < bh && gx >= 0 && gx < nx)
-        box[(q * bh + rr) * bw + cc] = src[q * g.fstride + (long long)bidx(gy, ny, bc) * g.pitch + gx];
+      if (rr >= 0 && rr < bh && gx >= 0 && gx < nx) box[(q * bh + rr) * bw + cc] = image(q, gx, bidx(gy, ny, bc));
     }
   }
 }

@@ -75,6 +75,7 @@ struct TileLaunch {
   const double* in;
   double* out;
   int ksteps;
+  int impl;    // 0 / 1 = fused_step_kernel (one CTA per tile), 2 = fused_tma_kernel (persistent CTAs fed by TMA, tilet.cuh)
   int window;  // Heun / RK4: 1 = 80 x 48 cells; two-field models also 2 = 48 x 40 (two CTAs per SM) and, RK4, 3 / 4 / 5 = 64 x 56 / 64 x 48 / 56 x 48
 };
 cudaError_t launch_fused_fhn(const Problem& pb, const TileLaunch& tl, cudaStream_t stream);
@@ -85,6 +86,22 @@ inline cudaError_t launch_fused(const Problem& pb, const TileLaunch& tl, cudaStr
                        : (pb.model == 1 ? launch_fused_karma(pb, tl, stream)
                                         : launch_fused_bocf(pb, tl, stream));
 }
+
+// tilet_kernels_*.cu: plan FUSED, implementation TMA (two-field models; windows 1 - 3; Euler: blocked steps only)
+cudaError_t launch_fusedt_fhn(const Problem& pb, const TileLaunch& tl, cudaStream_t stream);
+cudaError_t launch_fusedt_karma(const Problem& pb, const TileLaunch& tl, cudaStream_t stream);
+inline cudaError_t launch_fusedt(const Problem& pb, const TileLaunch& tl, cudaStream_t stream) {
+  return pb.model == 0 ? launch_fusedt_fhn(pb, tl, stream)
+                       : (pb.model == 1 ? launch_fusedt_karma(pb, tl, stream) : cudaErrorInvalidValue);
+}
+// window geometry (tile_dispatch.cuh FusedGeom) as the host needs it: output tile of window `win` at halo H
+inline void fused_tile_of(int win, int H, int& tw, int& th) {
+  const int ew = win == 2 ? 48 : (win == 3 || win == 4 || win == 7 ? 64 : (win == 5 ? 56 : 80));
+  const int eh = win == 2 ? 40 : (win == 3 || win == 7 ? 56 : 48);
+  tw = ew - 2 * H; th = eh - 2 * H;
+}
+bool fused_tma_supported(const Problem& pb, int window, int ksteps);
+constexpr long long kFusedTMinTiles = 3 * 148;   // AUTO: every persistent CTA has several tiles to pipeline
 
 // pair_kernels_*.cu: plan PAIR — two consecutive substeps per launch (pair.cuh): substep A (ka =
 // K_SELF or K_BASE) on tile + ring into shared memory (and into `mid` when not null), substep B (kb)

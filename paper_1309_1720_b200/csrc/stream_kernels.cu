@@ -374,6 +374,19 @@ bool stage_ring_supported(const Problem& pb, int kind) {
   return ntiles < (1LL << 31) && tma_available();
 }
 
+bool fused_tma_supported(const Problem& pb, int window, int ksteps) {
+  if (pb.nz > 1 || pb.nv > 2 || pb.integrator > I_RK4 || window < 1 || window > 7 || (window >= 4 && window <= 6)) return false;
+  if (pb.integrator == I_EULER && ksteps != kEulerBlock) return false;
+  if (pb.integrator != I_RK4 && window >= 3) return false;
+  const int ns = pb.integrator == I_RK4 ? 4 : (pb.integrator == I_HEUN ? 2 : ksteps);
+  const int H = pb.radius * ns;
+  int tw, th;
+  fused_tile_of(pb.integrator == I_EULER ? 1 : window, H, tw, th);
+  if (tw <= 0 || th <= 0 || pb.nx <= H + tw || pb.ny <= H + th) return false;   // one reflection maps every window index
+  const long long ntiles = (long long)((pb.nx + tw - 1) / tw) * ((pb.ny + th - 1) / th) * pb.batch;
+  return ntiles < (1LL << 31) && tma_available();
+}
+
 bool pair_tma_supported(const Problem& pb) {
   if (pb.nz > 1 || pb.integrator > I_RK4) return false;
   const long long ntiles = (long long)((pb.nx + 63) / 64) * ((pb.ny + 23) / 24) * pb.batch;

@@ -35,6 +35,14 @@ template <class MD, int H>
 struct FusedGeom<MD, H, 5> {
   using type = TileGeom<28, 12, 4>;  // 56 x 48 window, 336 threads
 };
+// the 64 x 56 window again with HALF the cells per thread (2 x 2) and twice the threads (64 registers): 28 warps
+// on the SM.  Measured on B200 (RK4): worse for FHN LAP9X4 (spills; 31 against 39 Gcell-step/s), better for
+// Karma LAP5, whose stage is bound by instruction issue: 1024^2 41 against 38.5 with one CTA per tile, and
+// 42 / 47 / 49.5 at 1024^2 / 2048^2 / 4096^2 with the TMA-fed persistent CTAs (tilet.cuh) against 38 / 40 / 41.
+template <class MD, int H>
+struct FusedGeom<MD, H, 7> {
+  using type = TileGeom<32, 28, 2>;  // 64 x 56 window, 896 threads
+};
 template <int VARIANT, int H, int WIN>
 struct FusedGeom<Model<M_BOCF, VARIANT>, H, WIN> {
   using type = TileGeom<24, 16, 2>;  // 48 x 32 window, 384 threads
@@ -109,6 +117,7 @@ cudaError_t fused_by_integrator(const Problem& pb, const TileLaunch& tl, cudaStr
         if (tl.window == 3) return fused_run<MD, STENCIL, I_RK4, 1, 3>(pb, tl, s);
         if (tl.window == 4) return fused_run<MD, STENCIL, I_RK4, 1, 4>(pb, tl, s);
         if (tl.window == 5) return fused_run<MD, STENCIL, I_RK4, 1, 5>(pb, tl, s);
+        if (tl.window == 7) return fused_run<MD, STENCIL, I_RK4, 1, 7>(pb, tl, s);
       }
       return fused_run<MD, STENCIL, I_RK4, 1>(pb, tl, s);
     case I_HEUN:

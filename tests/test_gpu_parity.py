@@ -100,7 +100,7 @@ def test_parity_fused_small_window(C, model, stencil, integ):
     auto = gpu_run(C, cfg, Z, 40, plan=(2, 0))
     assert maxabs(auto, large) <= 1e-12
     if integ == RK4:          # the three other one-CTA-per-SM windows, several ragged tiles each
-        for win in (3, 4, 5):
+        for win in (3, 4, 5, 7):
             other = gpu_run(C, cfg, Z, 40, plan=(2, win))
             assert maxabs(other, ref) <= tol(40) and maxabs(other, large) <= 1e-12
     else:
@@ -287,6 +287,37 @@ def test_fused_many_tiles_matches_stage_plan_and_oracle(C):
         assert maxabs(got, direct) <= 1e-12
         # the TMA-ring kernels run the same arithmetic per cell as the direct ones: bitwise equal
         assert np.array_equal(gpu_run(C, cfg, Z, 12, plan=RING), direct)
+
+
+@pytest.mark.parametrize("model", [FHN, KARMA])
+@pytest.mark.parametrize("stencil", [LAP5, LAP9X4, BOX9])
+@pytest.mark.parametrize("integ,windows", [(EULER, (0,)), (HEUN, (1, 2)), (RK4, (1, 2, 3, 7))])
+@pytest.mark.parametrize("bc", [0, 1])
+def test_fused_tma_implementation_bitwise_equal_to_fused(C, model, stencil, integ, windows, bc):
+    """Plan FUSED with persistent CTAs fed by TMA (parameter = window + 16 x 2): several tiles per CTA is not
+    needed for correctness — 251 x 170 x 2 members gives every window rim tiles on all four sides, a ragged
+    last column (odd width) and interior tiles; the ghost cells come from the box itself (no-flux) or from
+    global memory (periodic).  Same stage code as the one-CTA-per-tile kernel: the same bits; and the oracle."""
+    cfg, Z = make(model, 251, 170, stencil, integ, seed=23, boundary=bc, batch=2)
+    ref = O.step(model, Z, cfg.dx, cfg.dt, cfg.scheme, 13)
+    for win in windows:
+        got = gpu_run(C, cfg, Z, 13, plan=(2, win + 32))
+        assert maxabs(got, ref) <= tol(13)
+        assert np.array_equal(got, gpu_run(C, cfg, Z, 13, plan=(2, win + 16)))
+
+
+def test_fused_tma_limits_and_auto(C):
+    cfg, _ = make(FHN, 70, 45, LAP9X4, RK4)                       # smaller than window + halo: one reflection is not enough
+    with C.Context.from_config(cfg) as ctx:
+        with pytest.raises(C.CardiacError):
+            C.cardiac_set_plan(ctx.ctx, 2, 1 + 32)
+    cfg, _ = make(BOCF, 400, 400, LAP5, RK4)                      # two-field models only
+    with C.Context.from_config(cfg) as ctx:
+        with pytest.raises(C.CardiacError):
+            C.cardiac_set_plan(ctx.ctx, 2, 1 + 32)
+    cfg, Z = make(KARMA, 1100, 900, LAP5, RK4)                    # AUTO: TMA from 3 x 148 tiles; same bits as forced direct
+    auto = gpu_run(C, cfg, Z, 5, plan=(2, 0))
+    assert np.array_equal(auto, gpu_run(C, cfg, Z, 5, plan=(2, 16))) and np.array_equal(auto, gpu_run(C, cfg, Z, 5, plan=(2, 32)))
 
 
 @pytest.mark.parametrize("model,stencil,integ,bc", [(BOCF, LAP9X4, RK4, 0), (BOCF, LAP5, RK4, 1), (BOCF, BOX9, HEUN, 0),

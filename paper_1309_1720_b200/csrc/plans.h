@@ -176,7 +176,9 @@ inline ResidentShape resident_shape(const Problem& pb) {
   const int cmax = pb.batch <= 4 ? 16 : 8;   // 16: non-portable size, at most one such cluster per GPC
   for (int c = 1; c <= cmax; c *= 2) {
     const int slab = (pb.ny + c - 1) / c;
-    const size_t smem = 2 * (size_t)pb.nd * sp * ((size_t)slab + 2 * pb.radius) * sizeof(double);
+    // two stage buffers framed by the ghost ring + the two mbarriers of the ghost exchange
+    const size_t smem = 2 * (size_t)pb.nd * sp * ((size_t)slab + 2 * pb.radius) * sizeof(double) + 16;
+    if (c > 1 && slab < pb.radius) continue;   // the exchange reaches two CTAs up and down: slabs of at least r rows
     // fits, and one cell per thread where the grid is large enough to spread (a substep costs the
     // barrier plus the latency of one warp's instruction sequence, resident.cuh CPT)
     if (npx * slab <= cap && smem <= kResidentMaxSmem && (c == cmax || (pb.ny + 2 * c - 1) / (2 * c) < 4)) {

@@ -22,6 +22,7 @@
 #pragma once
 #include "stage.cuh"
 #include "tile.cuh"
+#include "tma.cuh"
 
 namespace cardiac {
 
@@ -54,24 +55,6 @@ CARDIAC_D unsigned cluster_rank() {
 CARDIAC_D void cluster_sync_all() {
   asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
-// The barrier between substeps orders SHARED memory only: every thread's stage results are st.shared to
-// its own CTA's buffer, and the readers are ld.shared::cluster of other CTAs, served by the shared
-// memory of the SM that owns the buffer — the only copy there is.  fence.acq_rel.cta (MEMBAR.ALL.CTA)
-// holds the arrive back until this thread's stores have been performed there; the arrive itself is
-// relaxed, which drops the GPU-scope MEMBAR of the release form (measured on B200, 64^2: FHN Euler
-// 0.98 -> 0.83 us per step, BOCF RK4 13.9 -> 11.5 us); the wait keeps its acquire.
-CARDIAC_D void cluster_sync_shared() {
-  asm volatile("fence.acq_rel.cta;\n\tbarrier.cluster.arrive.relaxed.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
-// the value at the same shared-memory offset as `p` in CTA `rank` of the cluster
-CARDIAC_D double ld_cluster(const double* p, unsigned rank) {
-  unsigned local = (unsigned)__cvta_generic_to_shared(p), remote;
-  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local), "r"(rank));
-  double v;
-  asm volatile("ld.shared::cluster.f64 %0, [%1];" : "=d"(v) : "r"(remote) : "memory");
-  return v;
-}
-
 // CPT = cells per thread and unit: 2 = an x-adjacent pair (128-bit shared-memory accesses); 1 = ONE cell
 // of the pair, the even warps taking the first and the odd warps the second cell of the same 32 pairs
 // (warp-uniform, so each branch keeps only its half of stencil_pair): a substep of a small grid is bound
@@ -86,64 +69,121 @@ struct ResidentEngine {
   static constexpr int NT = kResidentThreads;
   static constexpr int GX = 2;  // ghost columns kept on each side (>= r; keeps pairs 16-byte aligned)
 
-  static constexpr int GK = 2;  // ghost cells per thread decoded once
-  struct Ghost;
+  static constexpr int GK = 3;  // exchange duties per thread decoded once
+  struct Duty;
   struct Patch;
 
-
-  // The ghost ring of the slab [y0, y0 + rows): ghost columns -r..-1, nx..nx+r-1 of the own rows
-  // (source: the own row, reflected / wrapped column) and ghost rows y0-r..y0-1, y0+rows..y0+rows+r-1
-  // over the columns 0..nx-1 (source: the CTA that owns the grid row the index stands for).
-  // Entry e of that list -> offset of the ghost cell inside buffer 0, offset of its source, owner.
-  struct Ghost {
-    int dst, src;
-    unsigned owner;
+  // The ghost ring of a slab [y0, y0 + rows): ghost columns -r..-1, nx..nx+r-1 of the own rows (source: the own
+  // row, reflected / wrapped column) and ghost rows y0-r..y0-1, y0+rows..y0+rows+r-1 over the columns 0..nx-1
+  // (source: the CTA that owns the grid row the index reflects / wraps / continues to).  The ring is filled by
+  // the OWNER of the source cell (push): a duty = "copy the value at offset `src` of my buffer to offset `dst`
+  // of CTA `dest`'s buffer" (dest < 0: my own buffer, a plain shared-memory copy — the ghost columns).
+  struct Duty {
+    int dst, src, dest;   // dst < 0: none
   };
   struct Patch {
     double y[RK ? KP : 1][CPT][NV];
     double acc[RK ? KP : 1][CPT][NV];
     double g[KP][CPT][NG > 0 ? NG : 1];
     int off[KP];   // offset of the pair inside a shared field, -1 = no such pair (CPT = 1: or no such cell)
-    Ghost gh[GK];  // dst < 0: none
+    Duty du[GK];   // the first GK duties of this thread
+    int more;      // list position from which further duties are decoded on the fly (very wide grids), -1 = none
   };
-  CARDIAC_D static Ghost ghost_entry(const ResidentArgs<MD>& a, int e, int y0, int rows, unsigned rank) {
-    const int nx = a.g.nx, ny = a.g.ny, bc = a.g.boundary, sp = a.sp;
-    const int ncol = 2 * R * rows, nrow = 2 * R * nx;
-    const int q = e / (ncol + nrow), f = e - q * (ncol + nrow);
-    const int fo = q * a.sp * a.sr;
-    Ghost gh;
-    if (f < ncol) {
+  // number of CTAs that hold rows
+  CARDIAC_D static int active_ctas(const ResidentArgs<MD>& a) { return (a.g.ny + a.slab - 1) / a.slab; }
+  CARDIAC_D static int duty_count(const ResidentArgs<MD>& a, int rows) {
+    return rows > 0 ? ND * 2 * R * rows + 5 * ND * 2 * R * a.g.nx : 0;
+  }
+  // Entry e of the duty list of CTA `rank`: first the ghost columns of its own rows, then the ghost ROWS of the
+  // CTAs rank-2 .. rank+2 (wrapped on a periodic grid, clipped otherwise; with slabs of at least r rows no
+  // other CTA can need a row of this one) — such an entry is a duty iff this CTA owns the source row.
+  CARDIAC_D static Duty duty_entry(const ResidentArgs<MD>& a, int e, int y0, int rows, int rank) {
+    const int nx = a.g.nx, ny = a.g.ny, bc = a.g.boundary, sp = a.sp, fsz = a.sp * a.sr;
+    const int ncol = ND * 2 * R * rows, L = ND * 2 * R * nx;
+    Duty d;
+    d.dst = -1; d.src = 0; d.dest = -1;
+    if (e < ncol) {
+      const int q = e / (2 * R * rows), f = e - q * (2 * R * rows);
       const int k = f / rows, lr = f - k * rows + R;
       const int gx = k < R ? -1 - k : nx + (k - R);
-      gh.dst = fo + lr * sp + GX + gx;
-      gh.src = fo + lr * sp + GX + bidx(gx, nx, bc);
-      gh.owner = rank;
-    } else {
-      const int h = f - ncol, k = h / nx, gx = h - k * nx;
-      const int gy = k < R ? y0 - 1 - k : y0 + rows + (k - R);
-      const int gs = bidx(gy, ny, bc);          // the grid row it stands for
-      gh.owner = (unsigned)(gs / a.slab);
-      gh.dst = fo + (gy - y0 + R) * sp + GX + gx;
-      gh.src = fo + (gs - (int)gh.owner * a.slab + R) * sp + GX + gx;
+      d.dst = q * fsz + lr * sp + GX + gx;
+      d.src = q * fsz + lr * sp + GX + bidx(gx, nx, bc);
+      return d;
     }
-    return gh;
+    const int er = e - ncol, o = er / L, h = er - o * L;
+    const int ca = active_ctas(a);
+    auto target = [&](int oo) -> int {   // the CTA at offset oo - 2, -1 = none
+      int D = rank + oo - 2;
+      if (bc == B_PERIODIC) { D %= ca; if (D < 0) D += ca; }
+      return (D < 0 || D >= ca) ? -1 : D;
+    };
+    const int D = target(o);
+    if (D < 0) return d;
+    for (int oo = 0; oo < o; ++oo)
+      if (target(oo) == D) return d;   // the same CTA under a smaller offset (few CTAs on a periodic grid)
+    const int q = h / (2 * R * nx), f = h - q * (2 * R * nx), k = f / nx, gx = f - k * nx;
+    const int y0d = D * a.slab, rowsd = min(a.slab, ny - y0d);
+    const int gy = k < R ? y0d - 1 - k : y0d + rowsd + (k - R);
+    const int gs = bidx(gy, ny, bc);          // the grid row it stands for
+    if (gs / a.slab != rank) return d;
+    d.dst = q * fsz + (gy - y0d + R) * sp + GX + gx;
+    d.src = q * fsz + (gs - y0 + R) * sp + GX + gx;
+    d.dest = D;
+    return d;
   }
 
-  // Refill the ghost ring of buffer `b`.  Call after a cluster barrier (the interior of `b` is
-  // complete in every CTA); ends with a CTA barrier.  The first GK entries of every thread were
-  // decoded once (Patch::gh); longer lists (very wide grids) are decoded on the fly.
-  CARDIAC_D static void fill_ghosts(const ResidentArgs<MD>& a, double* __restrict__ b, int y0, int rows,
-                                    unsigned rank, const Patch& st) {
-    const int nghost = rows > 0 ? ND * 2 * R * (rows + a.g.nx) : 0;
+  // Complete the ghost ring of buffer `b` in every CTA (exchange number g = 0, 1, ... of this launch).  Call
+  // after a CTA barrier (the own interior of `b` is complete); ends with a CTA barrier.
+  // Ghost rows travel by st.async: the store lands in the destination CTA's shared memory and completes a
+  // transaction count on ITS mbarrier bar[g & 1]; a CTA waits for the 2 r nx n_d values of its own ring and
+  // for nobody else — no cluster-wide barrier and no fence between substeps (the async store carries its own
+  // release, the wait acquires at cluster scope).  Why two mbarriers: a neighbour that already has all of ITS
+  // ghost rows may run one exchange ahead and deliver exchange g+1 while this CTA still waits for another
+  // neighbour's exchange g; it cannot be two ahead, because exchange g+2 needs this CTA's rows of g+1.  Why no
+  // "buffer free" signal: a CTA pushes after its CTA barrier, i.e. when all of its threads have finished
+  // reading the buffer that exchange g+1 of its neighbours will overwrite, and those neighbours need its
+  // pushes before they can get there.
+  CARDIAC_D static void exchange(const ResidentArgs<MD>& a, double* __restrict__ b, uint64_t* bars, int g, int y0,
+                                 int rows, int rank, const Patch& st) {
+    uint64_t* const bar = bars + (g & 1);
+    if (rows > 0 && threadIdx.x == 0) mbar_arrive_expect_tx(bar, (unsigned)(ND * 2 * R * a.g.nx * sizeof(double)));
+    auto run_duty = [&](const Duty& d) {
+      const double v = b[d.src];
+      if (d.dest < 0) {
+        b[d.dst] = v;
+      } else {
+        unsigned raddr, rbar;
+        asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(raddr) : "r"(smem_u32(b + d.dst)), "r"(d.dest));
+        asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rbar) : "r"(smem_u32(bar)), "r"(d.dest));
+        asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.f64 [%0], %1, [%2];" ::"r"(raddr),
+                     "d"(v), "r"(rbar)
+                     : "memory");
+      }
+    };
 #pragma unroll
     for (int k = 0; k < GK; ++k)
-      if (st.gh[k].dst >= 0) b[st.gh[k].dst] = ld_cluster(b + st.gh[k].src, st.gh[k].owner);
-    for (int e = threadIdx.x + GK * NT; e < nghost; e += NT) {
-      const Ghost gh = ghost_entry(a, e, y0, rows, rank);
-      b[gh.dst] = ld_cluster(b + gh.src, gh.owner);
+      if (st.du[k].dst >= 0) run_duty(st.du[k]);
+    if (st.more >= 0) {
+      const int ne = duty_count(a, rows);
+      for (int e = st.more; e < ne; e += NT) {
+        const Duty d = duty_entry(a, e, y0, rows, rank);
+        if (d.dst >= 0) run_duty(d);
+      }
     }
-    __syncthreads();
-    if (STENCIL == S_BOX9) {   // corners: ghost columns of the ghost rows
+    if (rows > 0) {
+      const unsigned parity = (unsigned)(g >> 1) & 1u;
+      unsigned ok;
+      do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+      } while (!ok);
+    }
+    if (STENCIL == S_BOX9) {   // corners: ghost columns of the ghost rows (which have just arrived)
       const int nx = a.g.nx, bc = a.g.boundary, sp = a.sp, fsz = a.sp * a.sr;
       for (int e = threadIdx.x; e < ND * 2 * R * 2 * R && rows > 0; e += NT) {
         const int q = e / (4 * R * R), f = e - q * 4 * R * R, kr = f / (2 * R), kc = f - kr * 2 * R;
@@ -152,8 +192,8 @@ struct ResidentEngine {
         double* F = b + q * fsz;
         F[lr * sp + GX + gx] = F[lr * sp + GX + bidx(gx, nx, bc)];
       }
-      __syncthreads();
     }
+    __syncthreads();
   }
 
   // pair index of unit k of this thread, and (CPT = 1) which cell of the pair the thread owns
@@ -241,17 +281,17 @@ struct ResidentEngine {
   }
 
   template <int S>
-  CARDIAC_D static void stages_from(const ResidentArgs<MD>& a, double* __restrict__ sm, int& cur,
-                                    Patch& st, int y0, int rows, unsigned rank) {
+  CARDIAC_D static void stages_from(const ResidentArgs<MD>& a, double* __restrict__ sm, uint64_t* bars, int& cur,
+                                    int& g, Patch& st, int y0, int rows, unsigned rank) {
     if constexpr (S < NS) {
       const int fsz = a.sp * a.sr;
       double* c = sm + cur * ND * fsz;
       double* n = sm + (cur ^ 1) * ND * fsz;
       stage<S>(a, c, n, st);
-      cluster_sync_shared();
-      fill_ghosts(a, n, y0, rows, rank, st);
+      __syncthreads();
+      exchange(a, n, bars, g++, y0, rows, (int)rank, st);
       cur ^= 1;
-      stages_from<S + 1>(a, sm, cur, st, y0, rows, rank);
+      stages_from<S + 1>(a, sm, bars, cur, g, st, y0, rows, rank);
     }
   }
 
@@ -292,19 +332,32 @@ struct ResidentEngine {
         }
       }
     }
-    {
-      const int nghost = rows > 0 ? ND * 2 * R * (rows + nx) : 0;
+    {   // this thread's exchange duties: the first GK decoded once
+      const int ne = duty_count(a, rows);
+      int found = 0;
+      st.more = -1;
 #pragma unroll
-      for (int k = 0; k < GK; ++k) {
-        const int e = threadIdx.x + k * NT;
-        st.gh[k].dst = -1;
-        if (e < nghost) st.gh[k] = ghost_entry(a, e, y0, rows, rank);
+      for (int k = 0; k < GK; ++k) st.du[k].dst = -1;
+      for (int e = threadIdx.x; e < ne; e += NT) {
+        const Duty d = duty_entry(a, e, y0, rows, (int)rank);
+        if (d.dst < 0) continue;
+        if (found >= GK) { st.more = e; break; }
+#pragma unroll
+        for (int k = 0; k < GK; ++k)
+          if (k == found) st.du[k] = d;
+        ++found;
       }
     }
-    cluster_sync_all();
-    fill_ghosts(a, sm, y0, rows, rank, st);
-    int cur = 0;
-    for (long long n = 0; n < a.nsteps; ++n) stages_from<0>(a, sm, cur, st, y0, rows, rank);
+    uint64_t* const bars = reinterpret_cast<uint64_t*>(sm + 2 * ND * fsz);
+    if (threadIdx.x == 0) {
+      mbar_init(bars, 1);
+      mbar_init(bars + 1, 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    cluster_sync_all();   // the loads are done and every CTA's mbarriers exist before the first push
+    int cur = 0, g = 0;
+    exchange(a, sm, bars, g++, y0, rows, (int)rank, st);
+    for (long long n = 0; n < a.nsteps; ++n) stages_from<0>(a, sm, bars, cur, g, st, y0, rows, rank);
     // store the state: diffusing fields from the current shared buffer, gates from registers
     const double* c = sm + cur * ND * fsz;
 #pragma unroll

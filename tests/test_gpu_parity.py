@@ -154,14 +154,15 @@ def test_parity_persistent_edges(C, model, stencil, nx, ny, bc):
 @pytest.mark.parametrize("model,stencil,integ,n,batch,nsteps", [(FHN, LAP5, EULER, 64, 1, 6000), (KARMA, LAP9X4, RK4, 96, 4, 1500),
                                                                 (BOCF, LAP9X4, RK4, 128, 4, 800), (FHN, BOX9, HEUN, 100, 16, 1500)])
 def test_persistent_barrier_stress(C, model, stencil, integ, n, batch, nsteps):
-    """The barrier between substeps orders shared memory only (fence.acq_rel.cta + relaxed cluster
-    arrive + acquire wait, resident.cuh) and compute-sanitizer's racecheck is not available on the
-    GPU pool: a ghost row read before its owner's store had landed, or a buffer overwritten while a
-    neighbour still reads it, would make a long run depend on timing.  Thousands of substeps in one
-    launch (clusters of 16 and of 8, every cluster co-resident), repeated while another stream keeps
-    the other SMs and the L2 busy, and split into launches of other lengths: the same bits every
-    time, and the state still that of the stage-synchronous plan (a stale value is an O(1) error in
-    a cell, far above the roundoff between the two plans)."""
+    """Between substeps there is no cluster-wide barrier: ghost rows are pushed into the neighbours' shared
+    memory with st.async and each CTA waits on its own mbarrier (resident.cuh); a CTA may run one exchange
+    ahead of a neighbour.  compute-sanitizer's racecheck is not available on the GPU pool, so: a ghost row
+    used before it arrived, counted towards the wrong exchange, or a buffer overwritten while a neighbour's
+    rows were still being read would make a long run depend on timing.  Thousands of substeps in one launch
+    (clusters of 16 and of 8, every cluster co-resident), repeated while another stream keeps the other SMs
+    and the L2 busy, and split into launches of other lengths: the same bits every time, and the state still
+    that of the stage-synchronous plan (a stale value is an O(1) error in a cell, far above the roundoff
+    between the two plans)."""
     import torch
     cfg, Z = make(model, n, n, stencil, integ, batch=batch)
     ref = gpu_run(C, cfg, Z, nsteps, plan=PERSISTENT)

@@ -176,8 +176,8 @@ inline ResidentShape resident_shape(const Problem& pb) {
   const int cmax = pb.batch <= 4 ? 16 : 8;   // 16: non-portable size, at most one such cluster per GPC
   for (int c = 1; c <= cmax; c *= 2) {
     const int slab = (pb.ny + c - 1) / c;
-    // two stage buffers framed by the ghost ring + the two mbarriers of the ghost exchange
-    const size_t smem = 2 * (size_t)pb.nd * sp * ((size_t)slab + 2 * pb.radius) * sizeof(double) + 16;
+    // two stage buffers framed by the ghost ring + the two mbarriers and the row-duty table of the ghost exchange
+    const size_t smem = 2 * (size_t)pb.nd * sp * ((size_t)slab + 2 * pb.radius) * sizeof(double) + 16 + 256;
     if (c > 1 && slab < pb.radius) continue;   // the exchange reaches two CTAs up and down: slabs of at least r rows
     // fits, and one cell per thread where the grid is large enough to spread (a substep costs the
     // barrier plus the latency of one warp's instruction sequence, resident.cuh CPT)
@@ -189,20 +189,21 @@ inline ResidentShape resident_shape(const Problem& pb) {
   return rs;
 }
 inline bool resident_supported(const Problem& pb) { return resident_shape(pb).csize > 0; }
-// AUTO: measured on B200: a substep of the cluster-resident launch costs the barrier,
-// the ghost exchange and the latency of one warp's instruction sequence, which grows with the cells a
-// CTA holds; against the per-step launches of FUSED / STAGE it wins up to (batch 1, 16 CTAs) 180^2 for
-// FHN Euler, 120^2 for FHN RK4, 140^2 for Karma RK4, 128^2 for BOCF (one cell per thread) — expressed per
-// CTA so that it carries over to the 8-CTA clusters of larger batches — and only while every cluster is
-// resident at once (a GPC holds one cluster of 16, two of 8, four of 4: 17 members in clusters of 8 run
-// as two waves, 8.0 against 6.0 us per FHN RK4 step at 64^2).
+// AUTO: measured on B200: a substep of the cluster-resident launch costs the ghost
+// exchange (a remote store and the wait for the neighbours') and the latency of one warp's instruction
+// sequence, which grows with the cells a CTA holds; against the per-step launches of FUSED / STAGE it wins up
+// to (batch 1, 16 CTAs; round 2, push exchange) 192^2 for FHN Euler (1.36 against 1.69 us per step), 144^2 for
+// FHN RK4 (5.4 / 5.9), Karma RK4 (5.3 / 6.2) and BOCF RK4 (12.8 / 13.5) — expressed per CTA so that it carries
+// over to the 8-CTA clusters of larger batches — and only while every cluster is resident at once (a GPC holds
+// one cluster of 16, two of 8, four of 4: 17 members in clusters of 8 run as two waves, 8.0 against 6.0 us per
+// FHN RK4 step at 64^2).
 inline bool resident_preferred(const Problem& pb) {
   const ResidentShape rs = resident_shape(pb);
   if (rs.csize == 0) return false;
   const int max_clusters = rs.csize == 16 ? 4 : (rs.csize == 8 ? 16 : (rs.csize == 4 ? 32 : 144 / rs.csize));
   if (pb.batch > max_clusters) return false;
   const long long cells_per_cta = 2LL * ((pb.nx + 1) / 2) * rs.slab;
-  const long long limit = pb.nv > 2 ? 1024 : (pb.integrator == 0 ? 2048 : (pb.model == 0 ? 900 : 1200));
+  const long long limit = pb.nv > 2 ? 1300 : (pb.integrator == 0 ? 2400 : (pb.model == 0 ? 1300 : 1400));
   return cells_per_cta <= limit;
 }
 cudaError_t launch_resident_fhn(const Problem& pb, const ResidentLaunch& rl, cudaStream_t stream);

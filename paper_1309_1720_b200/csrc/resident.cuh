@@ -91,44 +91,59 @@ struct ResidentEngine {
   };
   // number of CTAs that hold rows
   CARDIAC_D static int active_ctas(const ResidentArgs<MD>& a) { return (a.g.ny + a.slab - 1) / a.slab; }
-  CARDIAC_D static int duty_count(const ResidentArgs<MD>& a, int rows) {
-    return rows > 0 ? ND * 2 * R * rows + 5 * ND * 2 * R * a.g.nx : 0;
+  // Row duties of CTA `rank`: the ghost ROWS of the CTAs rank-2 .. rank+2 (wrapped on a periodic grid, clipped
+  // otherwise; with slabs of at least r rows no other CTA can need a row of this one) whose source row this CTA
+  // owns.  At most kMaxRowDuties; written once per launch by one thread into shared memory as triples
+  // (destination CTA, offset of the ghost row in its buffer, offset of the source row in mine), field 0, column 0.
+  static constexpr int kMaxRowDuties = 5 * 2 * R;
+  CARDIAC_D static int build_row_duties(const ResidentArgs<MD>& a, int* tab, int y0, int rank) {
+    const int ny = a.g.ny, bc = a.g.boundary, sp = a.sp, ca = active_ctas(a);
+    auto target = [&](int oo) -> int {   // the CTA at offset oo - 2, -1 = none
+      int D = rank + oo - 2;
+      if (bc == B_PERIODIC) { D %= ca; if (D < 0) D += ca; }
+      return (D < 0 || D >= ca) ? -1 : D;
+    };
+    int n = 0;
+    for (int o = 0; o < 5; ++o) {
+      const int D = target(o);
+      bool dup = D < 0;
+      for (int oo = 0; oo < o && !dup; ++oo) dup = target(oo) == D;   // the same CTA under a smaller offset
+      if (dup) continue;
+      const int y0d = D * a.slab, rowsd = min(a.slab, ny - y0d);
+      for (int k = 0; k < 2 * R; ++k) {
+        const int gy = k < R ? y0d - 1 - k : y0d + rowsd + (k - R);
+        const int gs = bidx(gy, ny, bc);          // the grid row it stands for
+        if (gs / a.slab != rank) continue;
+        tab[3 * n] = D;
+        tab[3 * n + 1] = (gy - y0d + R) * sp + GX;
+        tab[3 * n + 2] = (gs - y0 + R) * sp + GX;
+        ++n;
+      }
+    }
+    return n;
   }
-  // Entry e of the duty list of CTA `rank`: first the ghost columns of its own rows, then the ghost ROWS of the
-  // CTAs rank-2 .. rank+2 (wrapped on a periodic grid, clipped otherwise; with slabs of at least r rows no
-  // other CTA can need a row of this one) — such an entry is a duty iff this CTA owns the source row.
-  CARDIAC_D static Duty duty_entry(const ResidentArgs<MD>& a, int e, int y0, int rows, int rank) {
-    const int nx = a.g.nx, ny = a.g.ny, bc = a.g.boundary, sp = a.sp, fsz = a.sp * a.sr;
-    const int ncol = ND * 2 * R * rows, L = ND * 2 * R * nx;
+  // Entry e of the duty list: first the ghost columns of the own rows (local copies), then nrd row duties x
+  // n_d fields x nx columns.  Every entry is a duty; thread t takes e = t, t + NT, ...
+  CARDIAC_D static int duty_count(const ResidentArgs<MD>& a, int rows, int nrd) {
+    return rows > 0 ? ND * (2 * R * rows + nrd * a.g.nx) : 0;
+  }
+  CARDIAC_D static Duty duty_entry(const ResidentArgs<MD>& a, const int* tab, int e, int rows) {
+    const int nx = a.g.nx, bc = a.g.boundary, sp = a.sp, fsz = a.sp * a.sr;
+    const int ncol = ND * 2 * R * rows;
     Duty d;
-    d.dst = -1; d.src = 0; d.dest = -1;
     if (e < ncol) {
       const int q = e / (2 * R * rows), f = e - q * (2 * R * rows);
       const int k = f / rows, lr = f - k * rows + R;
       const int gx = k < R ? -1 - k : nx + (k - R);
       d.dst = q * fsz + lr * sp + GX + gx;
       d.src = q * fsz + lr * sp + GX + bidx(gx, nx, bc);
+      d.dest = -1;
       return d;
     }
-    const int er = e - ncol, o = er / L, h = er - o * L;
-    const int ca = active_ctas(a);
-    auto target = [&](int oo) -> int {   // the CTA at offset oo - 2, -1 = none
-      int D = rank + oo - 2;
-      if (bc == B_PERIODIC) { D %= ca; if (D < 0) D += ca; }
-      return (D < 0 || D >= ca) ? -1 : D;
-    };
-    const int D = target(o);
-    if (D < 0) return d;
-    for (int oo = 0; oo < o; ++oo)
-      if (target(oo) == D) return d;   // the same CTA under a smaller offset (few CTAs on a periodic grid)
-    const int q = h / (2 * R * nx), f = h - q * (2 * R * nx), k = f / nx, gx = f - k * nx;
-    const int y0d = D * a.slab, rowsd = min(a.slab, ny - y0d);
-    const int gy = k < R ? y0d - 1 - k : y0d + rowsd + (k - R);
-    const int gs = bidx(gy, ny, bc);          // the grid row it stands for
-    if (gs / a.slab != rank) return d;
-    d.dst = q * fsz + (gy - y0d + R) * sp + GX + gx;
-    d.src = q * fsz + (gs - y0 + R) * sp + GX + gx;
-    d.dest = D;
+    const int er = e - ncol, i = er / (ND * nx), rem = er - i * (ND * nx), q = rem / nx, gx = rem - q * nx;
+    d.dest = tab[3 * i];
+    d.dst = q * fsz + tab[3 * i + 1] + gx;
+    d.src = q * fsz + tab[3 * i + 2] + gx;
     return d;
   }
 
@@ -143,8 +158,8 @@ struct ResidentEngine {
   // "buffer free" signal: a CTA pushes after its CTA barrier, i.e. when all of its threads have finished
   // reading the buffer that exchange g+1 of its neighbours will overwrite, and those neighbours need its
   // pushes before they can get there.
-  CARDIAC_D static void exchange(const ResidentArgs<MD>& a, double* __restrict__ b, uint64_t* bars, int g, int y0,
-                                 int rows, int rank, const Patch& st) {
+  CARDIAC_D static void exchange(const ResidentArgs<MD>& a, double* __restrict__ b, uint64_t* bars, int g, int rows,
+                                 int ne, const Patch& st) {
     uint64_t* const bar = bars + (g & 1);
     if (rows > 0 && threadIdx.x == 0) mbar_arrive_expect_tx(bar, (unsigned)(ND * 2 * R * a.g.nx * sizeof(double)));
     auto run_duty = [&](const Duty& d) {
@@ -163,12 +178,9 @@ struct ResidentEngine {
 #pragma unroll
     for (int k = 0; k < GK; ++k)
       if (st.du[k].dst >= 0) run_duty(st.du[k]);
-    if (st.more >= 0) {
-      const int ne = duty_count(a, rows);
-      for (int e = st.more; e < ne; e += NT) {
-        const Duty d = duty_entry(a, e, y0, rows, rank);
-        if (d.dst >= 0) run_duty(d);
-      }
+    if (st.more >= 0) {   // very wide grids: more than GK duties per thread, decoded on the fly
+      const int* tab = reinterpret_cast<const int*>(bars + 2);
+      for (int e = st.more; e < ne; e += NT) run_duty(duty_entry(a, tab, e, rows));
     }
     if (rows > 0) {
       const unsigned parity = (unsigned)(g >> 1) & 1u;
@@ -282,16 +294,16 @@ struct ResidentEngine {
 
   template <int S>
   CARDIAC_D static void stages_from(const ResidentArgs<MD>& a, double* __restrict__ sm, uint64_t* bars, int& cur,
-                                    int& g, Patch& st, int y0, int rows, unsigned rank) {
+                                    int& g, Patch& st, int rows, int ne) {
     if constexpr (S < NS) {
       const int fsz = a.sp * a.sr;
       double* c = sm + cur * ND * fsz;
       double* n = sm + (cur ^ 1) * ND * fsz;
       stage<S>(a, c, n, st);
       __syncthreads();
-      exchange(a, n, bars, g++, y0, rows, (int)rank, st);
+      exchange(a, n, bars, g++, rows, ne, st);
       cur ^= 1;
-      stages_from<S + 1>(a, sm, bars, cur, g, st, y0, rows, rank);
+      stages_from<S + 1>(a, sm, bars, cur, g, st, rows, ne);
     }
   }
 
@@ -332,32 +344,27 @@ struct ResidentEngine {
         }
       }
     }
-    {   // this thread's exchange duties: the first GK decoded once
-      const int ne = duty_count(a, rows);
-      int found = 0;
-      st.more = -1;
-#pragma unroll
-      for (int k = 0; k < GK; ++k) st.du[k].dst = -1;
-      for (int e = threadIdx.x; e < ne; e += NT) {
-        const Duty d = duty_entry(a, e, y0, rows, (int)rank);
-        if (d.dst < 0) continue;
-        if (found >= GK) { st.more = e; break; }
-#pragma unroll
-        for (int k = 0; k < GK; ++k)
-          if (k == found) st.du[k] = d;
-        ++found;
-      }
-    }
     uint64_t* const bars = reinterpret_cast<uint64_t*>(sm + 2 * ND * fsz);
+    int* const tab = reinterpret_cast<int*>(bars + 2);   // [0] = number of row duties, then the triples
     if (threadIdx.x == 0) {
       mbar_init(bars, 1);
       mbar_init(bars + 1, 1);
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+      tab[3 * kMaxRowDuties] = rows > 0 ? build_row_duties(a, tab, y0, (int)rank) : 0;
     }
     cluster_sync_all();   // the loads are done and every CTA's mbarriers exist before the first push
+    const int ne = duty_count(a, rows, tab[3 * kMaxRowDuties]);
+    st.more = -1;
+#pragma unroll
+    for (int k = 0; k < GK; ++k) {   // this thread's exchange duties: the first GK decoded once
+      const int e = threadIdx.x + k * NT;
+      st.du[k].dst = -1;
+      if (e < ne) st.du[k] = duty_entry(a, tab, e, rows);
+    }
+    if (threadIdx.x + GK * NT < ne) st.more = threadIdx.x + GK * NT;
     int cur = 0, g = 0;
-    exchange(a, sm, bars, g++, y0, rows, (int)rank, st);
-    for (long long n = 0; n < a.nsteps; ++n) stages_from<0>(a, sm, bars, cur, g, st, y0, rows, rank);
+    exchange(a, sm, bars, g++, rows, ne, st);
+    for (long long n = 0; n < a.nsteps; ++n) stages_from<0>(a, sm, bars, cur, g, st, rows, ne);
     // store the state: diffusing fields from the current shared buffer, gates from registers
     const double* c = sm + cur * ND * fsz;
 #pragma unroll

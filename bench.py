@@ -352,7 +352,14 @@ def measure_fp64(C, cfg_small, gpu_index=0):
         sampler.start()
         sustained = C.cardiac_measure_fp64_peak(ctx.ctx, 120000, 2)
         clocks = sampler.stop()
-    return {"dfma_per_s_burst": burst, "dfma_per_s_sustained": sustained,
+        # what an FP64 instruction costs a scheduler's issue port: DFMA rate with 0 / 2 / 4 independent integer
+        # instructions between the DFMAs (cycles = 2 x FP64 + others)
+        mhz = clocks.get("sm_mhz") or 1965.0
+        issue = {}
+        for m in (0, 2, 4):
+            r = C.cardiac_measure_fp64_issue(ctx.ctx, m, 4000, 3)
+            issue[str(m)] = {"dfma_per_s": r, "cycles_per_dfma_per_scheduler": 148 * 4 * 32 * mhz * 1e6 / r}
+    return {"dfma_per_s_burst": burst, "dfma_per_s_sustained": sustained, "issue_port_probe": issue,
             "tflops_burst": 2 * burst / 1e12, "tflops_sustained": 2 * sustained / 1e12,
             "nominal_tflops": FP64_NOMINAL_TFLOPS, "clocks_sustained": clocks,
             "how": "cardiac_measure_fp64_peak (include/cardiac_diag.h): 148 x 4 CTAs x 256 threads x 8 independent "

@@ -69,7 +69,7 @@ enum {
   CARDIAC_PLAN_FUSED      = 2, /* all substeps of one time step (or several Euler steps) on chip,
                                   overlapped tiles, one launch                                  */
   CARDIAC_PLAN_PERSISTENT = 3, /* ONE launch for all nsteps: each batch member resident in the shared
-                                  memory of a thread-block cluster (<= 8 CTAs), ghost rows exchanged
+                                  memory of a thread-block cluster (<= 16 CTAs), ghost rows pushed
                                   through distributed shared memory; grids up to C x 4096 cells
                                   (4-field model: C x 2048), C = 16 CTAs for batches of up to 4
                                   members, else 8; Euler, Heun, RK4                             */
@@ -129,13 +129,22 @@ int cardiac_get_params(const cardiac_ctx*, double* p, int n);
  * NULL = legacy default stream) for all subsequent work. */
 int cardiac_set_stream(cardiac_ctx*, void* cuda_stream);
 
-/* Choose the execution plan (CARDIAC_PLAN_*).  CARDIAC_ERR_INVALID if the plan does not support
- * the context's (model, scheme, size). `param` is plan specific: FUSED + Euler = time steps per
- * launch (0 = default); FUSED + Heun/RK4 = window (0 = by size, 1 = 80x48 cells, one CTA per SM,
- * 2 = 48x40 cells, two CTAs per SM, two-field models only, 3 / 4 / 5 = 64x56 / 64x48 / 56x48 cells, two-field models with RK4); STAGE = kernel implementation (0 = by size, 1 = DIRECT: every thread loads
- * its own operands, 2 = RING: persistent CTAs fed by a TMA shared-memory ring; same results
- * bitwise); PAIR, PERSISTENT: 0.  AUTO: PERSISTENT below ~120x120 .. 180x180 cells per member (by model and integrator; batches of up to 4 members, half of that up to 16), FUSED for the
- * two-field models, PAIR for the four-field model with RK4 from 1536^2 cells (Heun: 12 Mi), else STAGE. */
+/* Choose the execution plan (CARDIAC_PLAN_*).  CARDIAC_ERR_INVALID if the plan does not support the context's
+ * (model, scheme, size).  Every plan and implementation gives the same numbers (bitwise between implementations of
+ * a plan; to roundoff between plans).  `param` is plan specific:
+ *   STAGE      0 = by size, 1 = DIRECT (every thread loads its own operands), 2 = RING (persistent CTAs fed by a TMA
+ *              shared-memory ring)
+ *   PAIR       0 = by size, 1 = DIRECT, 2 = TMA (persistent CTAs, operands by box copies one tile ahead)
+ *   FUSED      Euler: time steps per launch (0 = default 4, or 1);  Heun / RK4: window + 16 x implementation with
+ *              window 0 = by size, 1 = 80x48 cells (one CTA per SM), 2 = 48x40 (two CTAs per SM; two-field models),
+ *              3 / 4 / 5 = 64x56 / 64x48 / 56x48 and 7 = 64x56 on 896 threads (two-field models, RK4), and
+ *              implementation 0 = by size, 1 = one CTA per tile, 2 = TMA (persistent CTAs whose windows arrive one
+ *              tile ahead; two-field models, windows 1, 2, 3, 7, grids larger than window + halo)
+ *   PERSISTENT 0
+ * AUTO: PERSISTENT below ~144x144 .. 192x192 cells per member (by model and integrator; batches of up to 4 members,
+ * half of that up to 16); FUSED for the two-field models (TMA implementation from ~450 tiles) and for a 4-field grid
+ * that is one wave of its tiles; PAIR (TMA) for the 4-field model with RK4 from 1024^2 cells (Heun: 12 Mi); else
+ * STAGE. */
 int cardiac_set_plan(cardiac_ctx*, int plan, int param);
 
 /* The plan that cardiac_step will use (resolved from AUTO). */

@@ -41,6 +41,14 @@ int cardiac_time_steps(cardiac_ctx*, long long nsteps, int reps, float* ms_total
  * iters >= 1, reps >= 1. */
 int cardiac_measure_fp64_peak(cardiac_ctx*, int iters, int reps, double* dfma_per_s);
 
+/* The same measurement with `int_per_dfma` (0, 2 or 4) independent integer instructions issued between the
+ * DFMAs of four chains per thread: what an FP64 instruction costs a scheduler's ISSUE port.  On B200 the
+ * rates come out as 1 / (2 + int_per_dfma) DFMA per cycle and scheduler — an FP64 instruction holds the port
+ * for two cycles and nothing else issues meanwhile — so the bound of the exp-heavy ionic kernels
+ * is 2 x (FP64 instructions) + (all other instructions), which bench.py reports beside
+ * the FP64-pipe fraction. */
+int cardiac_measure_fp64_issue(cardiac_ctx*, int iters, int reps, int int_per_dfma, double* dfma_per_s);
+
 #ifdef __cplusplus
 }
 #endif

@@ -38,7 +38,8 @@ EXPORTS = [
     "cardiac_last_error", "cardiac_destroy",
 ]
 # include/cardiac_diag.h: diagnostics for tests and bench.py, not part of the product boundary
-DIAG_EXPORTS = ["cardiac_probe", "cardiac_launch_count", "cardiac_time_steps", "cardiac_measure_fp64_peak"]
+DIAG_EXPORTS = ["cardiac_probe", "cardiac_launch_count", "cardiac_time_steps", "cardiac_measure_fp64_peak",
+                "cardiac_measure_fp64_issue"]
 
 
 class CardiacError(RuntimeError):
@@ -76,6 +77,7 @@ _sig = {
     "cardiac_launch_count": (_ll, [_vp]),
     "cardiac_time_steps": (_i, [_vp, _ll, _i, ctypes.POINTER(ctypes.c_float)]),
     "cardiac_measure_fp64_peak": (_i, [_vp, _i, _i, _dp]),
+    "cardiac_measure_fp64_issue": (_i, [_vp, _i, _i, _i, _dp]),
     "cardiac_last_error": (ctypes.c_char_p, [_vp]),
     "cardiac_destroy": (None, [_vp]),
 }
@@ -219,6 +221,13 @@ def cardiac_measure_fp64_peak(ctx, iters: int = 2000, reps: int = 5) -> float:
     """Thread-level DFMA instructions per second of the context's device (include/cardiac_diag.h)."""
     v = ctypes.c_double(0.0)
     _check(ctx, _lib.cardiac_measure_fp64_peak(ctx, iters, reps, ctypes.byref(v)))
+    return float(v.value)
+
+
+def cardiac_measure_fp64_issue(ctx, int_per_dfma: int, iters: int = 4000, reps: int = 3) -> float:
+    """Thread-level DFMA per second with int_per_dfma integer instructions between them (cardiac_diag.h)."""
+    v = ctypes.c_double(0.0)
+    _check(ctx, _lib.cardiac_measure_fp64_issue(ctx, iters, reps, int_per_dfma, ctypes.byref(v)))
     return float(v.value)
 
 

@@ -134,6 +134,14 @@ int auto_plan(const Problem& pb) {
   // RK4 1536^2 +2 %, 2048^2 +6 %, 4096^2 +15 %, 8192^2 +19 % over STAGE, behind at
   // 1024^2; Heun +2 % at 4096^2, behind at 2048^2)
   if (pb.model == CARDIAC_BOCF) {
+    // a grid that is ONE wave of the 4-field model's fused tiles (48 x 32 window) costs one CTA lifetime per time
+    // step instead of four launch-bound stage launches (round 2, LAP9X4 RK4: 256^2 9.6 against 14.4 us per step;
+    // two waves already lose: 362^2 18.5 against 16.5)
+    if (pb.integrator == I_RK4) {
+      const int H = pb.radius * 4, tw = 48 - 2 * H, th = 32 - 2 * H;
+      if (tw > 0 && th > 0 && (long long)((pb.nx + tw - 1) / tw) * ((pb.ny + th - 1) / th) * pb.batch <= 148)
+        return CARDIAC_PLAN_FUSED;
+    }
     const long long cells = (long long)pb.nx * pb.ny * pb.batch;
     if ((pb.integrator == I_RK4 && cells >= kPairMinCellsRK4) || (pb.integrator == I_HEUN && cells >= kPairMinCellsHeun))
       return CARDIAC_PLAN_PAIR;
@@ -776,7 +784,20 @@ int cardiac_time_steps(cardiac_ctx* c, long long nsteps, int reps, float* ms_tot
   return CARDIAC_OK;
 }
 
+namespace {
+int measure_dfma(cardiac_ctx* c, int iters, int reps, int int_per_dfma, double* dfma_per_s);
+}
 int cardiac_measure_fp64_peak(cardiac_ctx* c, int iters, int reps, double* dfma_per_s) {
+  return measure_dfma(c, iters, reps, -1, dfma_per_s);
+}
+int cardiac_measure_fp64_issue(cardiac_ctx* c, int iters, int reps, int int_per_dfma, double* dfma_per_s) {
+  if (c && int_per_dfma != 0 && int_per_dfma != 2 && int_per_dfma != 4)
+    return fail(c, CARDIAC_ERR_INVALID, "int_per_dfma must be 0, 2 or 4");
+  return measure_dfma(c, iters, reps, int_per_dfma, dfma_per_s);
+}
+namespace {
+// int_per_dfma < 0: the 8-chain peak kernel; else the 4-chain kernel with that many integer instructions per DFMA
+int measure_dfma(cardiac_ctx* c, int iters, int reps, int int_per_dfma, double* dfma_per_s) {
   if (!c) return CARDIAC_ERR_INVALID;
   if (!dfma_per_s || iters < 1 || reps < 1) return fail(c, CARDIAC_ERR_INVALID, "bad arguments");
   DeviceGuard guard(c->device);
@@ -791,7 +812,9 @@ int cardiac_measure_fp64_peak(cardiac_ctx* c, int iters, int reps, double* dfma_
   float best = 0.f;
   for (int r = 0; r <= reps && e == cudaSuccess; ++r) {   // r = 0: warm-up
     e = cudaEventRecord(e0, c->stream);
-    if (e == cudaSuccess) e = launch_dfma_peak(sink, blocks, iters, c->stream);
+    if (e == cudaSuccess)
+      e = int_per_dfma < 0 ? launch_dfma_peak(sink, blocks, iters, c->stream)
+                           : launch_dfma_mix(sink, blocks, iters, int_per_dfma, c->stream);
     if (e == cudaSuccess) e = cudaEventRecord(e1, c->stream);
     if (e == cudaSuccess) e = cudaEventSynchronize(e1);
     float ms = 0.f;
@@ -803,10 +826,12 @@ int cardiac_measure_fp64_peak(cardiac_ctx* c, int iters, int reps, double* dfma_
   if (e1) cudaEventDestroy(e1);
   cudaFree(sink);
   if (e != cudaSuccess) return fail_cuda(c, e, "fp64 peak");
-  const double n = (double)blocks * kDfmaThreads * kDfmaChains * kDfmaUnroll * (double)iters;
+  const double per_thread = int_per_dfma < 0 ? (double)kDfmaChains * kDfmaUnroll : (double)kDfmaMixChains * kDfmaMixUnroll;
+  const double n = (double)blocks * kDfmaThreads * per_thread * (double)iters;
   *dfma_per_s = n / ((double)best * 1e-3);
   return CARDIAC_OK;
 }
+}  // namespace
 
 const char* cardiac_last_error(const cardiac_ctx* c) {
   return c ? c->err.c_str() : g_create_error.c_str();

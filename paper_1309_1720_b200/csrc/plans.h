@@ -225,5 +225,9 @@ cudaError_t launch_probe(const Problem& pb, int what, const double* in, double* 
 // kDfmaChains independent chains of iters x kDfmaUnroll DFMAs; one double per thread is stored to `sink`
 constexpr int kDfmaThreads = 256, kDfmaChains = 8, kDfmaUnroll = 64;
 cudaError_t launch_dfma_peak(double* sink, int blocks, int iters, cudaStream_t stream);
+// ... four chains of iters x kDfmaMixUnroll DFMAs per thread with int_per_dfma (0, 2 or 4) independent integer
+// instructions in between (cardiac_measure_fp64_issue)
+constexpr int kDfmaMixChains = 4, kDfmaMixUnroll = 16;
+cudaError_t launch_dfma_mix(double* sink, int blocks, int iters, int int_per_dfma, cudaStream_t stream);
 
 }  // namespace cardiac

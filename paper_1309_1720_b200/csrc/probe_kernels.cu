@@ -54,10 +54,39 @@ __global__ void __launch_bounds__(256, 4) dfma_peak_kernel(double* __restrict__ 
   sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
 }
 
+// The same with M independent integer instructions (a LOP3 and an add on four separate chains) issued
+// between the DFMAs of a thread's four chains: does an FP64 instruction share its issue slot?  (It does not:
+// measured 2.0 / 3.7 / 6.1 cycles per DFMA and scheduler for 0 / 2 / 4 integer instructions per DFMA, i.e.
+// cycles = 2 x FP64 + 1 x others — DESIGN.md "FP64 issue".)
+template <int M>
+__global__ void __launch_bounds__(256, 4) dfma_mix_kernel(double* __restrict__ sink, int iters, double a, double b, int ia) {
+  double x0 = threadIdx.x * 1e-3, x1 = x0 + 0.1, x2 = x0 + 0.2, x3 = x0 + 0.3;
+  int i0 = threadIdx.x, i1 = i0 + 1, i2 = i0 + 2, i3 = i0 + 3;
+#pragma unroll 1
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 16; ++u) {
+      x0 = fma(x0, a, b); if (M >= 1) i0 = (i0 ^ ia) + 0x1234; if (M >= 2) i1 = (i1 ^ ia) + 0x4321;
+      x1 = fma(x1, a, b); if (M >= 1) i2 = (i2 ^ ia) + 0x1234; if (M >= 2) i3 = (i3 ^ ia) + 0x4321;
+      x2 = fma(x2, a, b); if (M >= 1) i0 = (i0 ^ ia) + 0x1111; if (M >= 2) i1 = (i1 ^ ia) + 0x2222;
+      x3 = fma(x3, a, b); if (M >= 1) i2 = (i2 ^ ia) + 0x3333; if (M >= 2) i3 = (i3 ^ ia) + 0x5555;
+    }
+  }
+  sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + (double)((i0 + i1) + (i2 + i3));
+}
+
 }  // namespace
 
 cudaError_t launch_dfma_peak(double* sink, int blocks, int iters, cudaStream_t s) {
   dfma_peak_kernel<<<blocks, kDfmaThreads, 0, s>>>(sink, iters, 0.999999, 1e-7);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_dfma_mix(double* sink, int blocks, int iters, int int_per_dfma, cudaStream_t s) {
+  if (int_per_dfma == 0) dfma_mix_kernel<0><<<blocks, kDfmaThreads, 0, s>>>(sink, iters, 0.999999, 1e-7, 0x55);
+  else if (int_per_dfma == 2) dfma_mix_kernel<1><<<blocks, kDfmaThreads, 0, s>>>(sink, iters, 0.999999, 1e-7, 0x55);
+  else if (int_per_dfma == 4) dfma_mix_kernel<2><<<blocks, kDfmaThreads, 0, s>>>(sink, iters, 0.999999, 1e-7, 0x55);
+  else return cudaErrorInvalidValue;
   return cudaGetLastError();
 }
 

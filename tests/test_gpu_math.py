@@ -80,3 +80,19 @@ def test_reaction_matches_oracle_pointwise(C, model, variant):
     ref = np.array([O.reaction(model, zi, variant=variant) for zi in z])
     scale = np.maximum(1.0, np.abs(ref))
     assert np.max(np.abs(got - ref) / scale) <= 2e-13
+
+
+def test_fp64_peak_and_issue_probe(C):
+    """The measured FP64 peak (include/cardiac_diag.h) is within reach of the nominal 148 x 64 x 1.965 GHz, and an
+    FP64 instruction does not share its issue slot: each integer instruction between two DFMAs costs about one
+    more cycle (the model behind DESIGN.md "FP64 issue")."""
+    cfg = W.make_config("probe", W.FHN, 8, W.LAP5, W.EULER, 0)
+    with C.Context.from_config(cfg) as ctx:
+        peak = C.cardiac_measure_fp64_peak(ctx.ctx, 2000, 3)
+        r = [C.cardiac_measure_fp64_issue(ctx.ctx, m, 2000, 3) for m in (0, 2, 4)]
+        with pytest.raises(C.CardiacError):
+            C.cardiac_measure_fp64_issue(ctx.ctx, 3, 10, 1)
+    nominal = 148 * 64 * 1.965e9
+    assert 0.6 * nominal < peak <= 1.02 * nominal
+    assert 0.8 * peak < r[0] <= 1.05 * peak
+    assert r[0] > 1.4 * r[1] and r[1] > 1.3 * r[2]      # 2 : ~3.7 : ~6 cycles per DFMA

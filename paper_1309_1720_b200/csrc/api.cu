@@ -547,7 +547,8 @@ int cardiac_set_plan(cardiac_ctx* c, int plan, int param) {
   if (resolved == CARDIAC_PLAN_STAGE) {
     if (param < 0 || param > 2)
       return fail(c, CARDIAC_ERR_INVALID, "STAGE: parameter must be 0 (auto), 1 (direct) or 2 (TMA ring)");
-    if (param == 2 && c->pb.nz > 1) return fail(c, CARDIAC_ERR_INVALID, "the TMA-ring stage kernels are 2-D only");
+    if (param == 2 && c->pb.nz > 1 && !stage_ring3d_supported(c->pb, K_SELF))
+      return fail(c, CARDIAC_ERR_INVALID, "the TMA-ring stage kernels are not available for this 3-D context");
     rparam = param;
   } else if (c->pb.nz > 1) {
     return fail(c, CARDIAC_ERR_INVALID, "3-D contexts run plan STAGE only");

@@ -58,6 +58,9 @@ cudaError_t launch_stage(const Problem& pb, const StageLaunch& st, cudaStream_t 
 bool stage_ring_supported(const Problem& pb, int kind);
 cudaError_t launch_stage_ring(const Problem& pb, const StageLaunch& st, cudaStream_t stream);
 constexpr long long kRingMinCells = 1 << 20;  // AUTO: below this the persistent grid has too few tiles per CTA
+// stream3d_kernels.cu: ... for 3-D grids: persistent CTAs marching along z, planes of the diffusing fields by TMA
+bool stage_ring3d_supported(const Problem& pb, int kind);
+cudaError_t launch_stage_ring3d(const Problem& pb, const StageLaunch& st, cudaStream_t stream);
 
 // jvp: J[b-1] = (Z[b] - Z[0]) / eps, pitched state -> dense output
 cudaError_t launch_jvp(const Problem& pb, const double* state, double eps, double* dst_dense,

@@ -319,6 +319,10 @@ cudaError_t launch_stage(const Problem& pb, const StageLaunch& st, cudaStream_t 
   // FP64 pipe or moves few bytes per cell; the TMA ring wins on the one stage that is purely
   // HBM-bound and operand-heavy — the last RK4 stage of the 4-field model (16 doubles in, 4 out per
   // cell; 6.3 TB/s = 96 % of the measured copy bandwidth, against 5.9 TB/s direct).
+  // 3-D: the z-marching TMA ring (stream3d_kernels.cu) only where forced — measured slower than the direct
+  // kernels at 256^3 for every model and stencil (8 - 16 warps per SM cannot hide its own shared-memory and FP64
+  // latencies)
+  if (pb.nz > 1 && pb.stage_impl == 2 && stage_ring3d_supported(pb, st.kind)) return launch_stage_ring3d(pb, st, stream);
   const long long cells = (long long)pb.nx * pb.ny * pb.batch;
   const bool ring_auto = st.kind == K_RK4F && pb.nv >= 4 && cells >= kRingMinCells;
   if (pb.stage_impl != 1 && (pb.stage_impl == 2 || ring_auto) && stage_ring_supported(pb, st.kind))

@@ -325,8 +325,8 @@ EncodeTiledFn encoder() {
 
 struct MapKey {
   const void* base;
-  int nx, ny, nf, batch, pitch, bw, bh;
-  long long fstride, bstride;
+  int nx, ny, nz, nf, batch, pitch, bw, bh;   // nz = 0: the 4-D view of a 2-D grid
+  long long zstride, fstride, bstride;
   bool operator==(const MapKey& o) const { return std::memcmp(this, &o, sizeof(MapKey)) == 0; }
 };
 struct MapEntry {
@@ -355,6 +355,35 @@ cudaError_t tensor_map_4d(const double* base, const Problem& pb, int nf, int bw,
   const cuuint32_t estr[4] = {1, 1, 1, 1};
   CUtensorMap m;
   CUresult r = enc(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double*>(base), gdim, gstr, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                   CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+  if (cache.size() >= 256) cache.clear();
+  cache.push_back({k, m});
+  *out = m;
+  return cudaSuccess;
+}
+
+// 5-D view (x, y, z, field, batch member) of a 3-D grid; box = bw x bh x 1 x nf x 1 (one plane)
+cudaError_t tensor_map_5d(const double* base, const Problem& pb, int nf, int bw, int bh, CUtensorMap* out) {
+  static std::mutex mu;
+  static std::vector<MapEntry> cache;
+  MapKey k;
+  std::memset(&k, 0, sizeof(k));
+  k.base = base; k.nx = pb.nx; k.ny = pb.ny; k.nz = pb.nz; k.nf = nf; k.batch = pb.batch; k.pitch = pb.pitch;
+  k.bw = bw; k.bh = bh; k.zstride = pb.zstride; k.fstride = pb.fstride; k.bstride = pb.bstride;
+  std::lock_guard<std::mutex> lock(mu);
+  for (const MapEntry& e : cache)
+    if (e.key == k) { *out = e.map; return cudaSuccess; }
+  EncodeTiledFn enc = encoder();
+  if (!enc) return cudaErrorNotSupported;
+  const cuuint64_t gdim[5] = {(cuuint64_t)pb.nx, (cuuint64_t)pb.ny, (cuuint64_t)pb.nz, (cuuint64_t)nf, (cuuint64_t)pb.batch};
+  const cuuint64_t gstr[4] = {(cuuint64_t)pb.pitch * 8, (cuuint64_t)pb.zstride * 8, (cuuint64_t)pb.fstride * 8,
+                              (cuuint64_t)pb.bstride * 8};
+  const cuuint32_t box[5] = {(cuuint32_t)bw, (cuuint32_t)bh, 1, (cuuint32_t)nf, 1};
+  const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+  CUtensorMap m;
+  CUresult r = enc(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, const_cast<double*>(base), gdim, gstr, box, estr,
                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;

@@ -73,10 +73,20 @@ CARDIAC_D void tma_load_4d(void* dst, const CUtensorMap* tm, int c0, int c1, int
       "l"(reinterpret_cast<uint64_t>(tm)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar))
       : "memory");
 }
+CARDIAC_D void tma_load_5d(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, int c3, int c4,
+                           uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.5d.shared::cluster.global.mbarrier::complete_tx::bytes "
+      "[%0], [%1, {%2, %3, %4, %5, %6}], [%7];" ::"r"(smem_u32(dst)),
+      "l"(reinterpret_cast<uint64_t>(tm)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(smem_u32(bar))
+      : "memory");
+}
 // ------------------------------------------------------------------ host
 // 4-D view (x, y, field, batch member) of `nf` fields starting at `base` (a field of the pitched state
 // buffers of `pb`), box = bw x bh x nf x 1; out-of-range elements are zero-filled.  Cached by value.
 cudaError_t tensor_map_4d(const double* base, const Problem& pb, int nf, int bw, int bh, CUtensorMap* out);
+// 5-D view (x, y, z, field, batch member) of a 3-D grid, box = bw x bh x 1 x nf x 1 (one plane)
+cudaError_t tensor_map_5d(const double* base, const Problem& pb, int nf, int bw, int bh, CUtensorMap* out);
 bool tma_available();   // the driver exports cuTensorMapEncodeTiled
 
 }  // namespace cardiac

@@ -36,8 +36,11 @@ def make(model, nx, ny, nz, stencil, integ, batch=1, seed=13, **kw):
     return cfg, W.initial_state(cfg)
 
 
-def gpu_run(C, cfg, Z, nsteps, chunks=None):
-    with C.Context.from_config(cfg) as ctx:
+DIRECT, RING = 1, 2     # plan STAGE: every thread loads its operands / z-marching persistent CTAs fed by a TMA ring
+
+
+def gpu_run(C, cfg, Z, nsteps, chunks=None, impl=0):
+    with C.Context.from_config(cfg, plan=1 if impl else 0, plan_param=impl) as ctx:
         assert ctx.plan == 1                                   # 3-D runs the stage-synchronous plan
         ctx.set_state(np.ascontiguousarray(Z))
         for n in (chunks or [nsteps]):
@@ -58,14 +61,29 @@ CASES += [(BOCF, s, i) for s in (LAP5, LAP9X4) for i in (RL, IE)]
 def test_parity_3d_one_and_fifty_steps(C, model, stencil, integ):
     # 141 x 27 x 7: interior blocks (x, y and z) as well as rim blocks on every face, odd width
     cfg, Z = make(model, 141, 27, 7, stencil, integ)
-    got1 = gpu_run(C, cfg, Z, 1)
+    got1 = gpu_run(C, cfg, Z, 1, impl=DIRECT)
     ref1 = O.step3d(model, Z, cfg.dx, cfg.dt, cfg.scheme, 1, omp=True)
     assert maxabs(got1, ref1) <= TOL_1
-    got = gpu_run(C, cfg, Z, 50)
+    got = gpu_run(C, cfg, Z, 50, impl=DIRECT)
     ref = O.step3d(model, ref1, cfg.dx, cfg.dt, cfg.scheme, 49, omp=True)
     assert np.all(np.isfinite(got))
     assert maxabs(got, ref) <= tol(50)
     assert maxabs(got, Z) > 1e-6
+    if integ in (EULER, HEUN, RK4):     # the TMA ring marching along z: the same arithmetic per cell, the same bits
+        assert np.array_equal(gpu_run(C, cfg, Z, 50, impl=RING), got)
+
+
+@pytest.mark.parametrize("model,stencil,nx,ny,nz,bc", [(FHN, LAP9X4, 200, 70, 75, 0), (KARMA, LAP5, 130, 19, 40, 1),
+                                                       (BOCF, LAP9X4, 67, 9, 33, 0), (FHN, LAP5, 64, 8, 32, 1),
+                                                       (FHN, LAP9X4, 65, 17, 5, 1)])
+def test_parity_3d_ring_chunks_and_tiles(C, model, stencil, nx, ny, nz, bc):
+    """The z-marching ring on grids of several 64 x 8 tiles and more than one chunk of 32 planes (75 = 32 + 32 + 11),
+    exactly one tile and one chunk, fewer planes than ring slots, ragged tiles, batch of 2: against the oracle and
+    bitwise against the direct kernels."""
+    cfg, Z = make(model, nx, ny, nz, stencil, RK4, boundary=bc, batch=2)
+    got = gpu_run(C, cfg, Z, 6, impl=RING)
+    assert np.array_equal(got, gpu_run(C, cfg, Z, 6, impl=DIRECT))
+    assert maxabs(got, O.step3d(model, Z, cfg.dx, cfg.dt, cfg.scheme, 6, omp=True)) <= tol(6)
 
 
 @pytest.mark.parametrize("model,stencil,nx,ny,nz,bc", [(FHN, LAP5, 3, 3, 3, 0), (KARMA, LAP9X4, 5, 5, 5, 0),
@@ -74,9 +92,10 @@ def test_parity_3d_one_and_fifty_steps(C, model, stencil, integ):
 def test_parity_3d_edges_and_periodic(C, model, stencil, nx, ny, nz, bc):
     """Minimum sizes 2r+1 in every direction (every arm reflects), thin slabs, periodic wrap in z."""
     cfg, Z = make(model, nx, ny, nz, stencil, RK4, boundary=bc)
-    got = gpu_run(C, cfg, Z, 20)
+    got = gpu_run(C, cfg, Z, 20, impl=DIRECT)
     ref = O.step3d(model, Z, cfg.dx, cfg.dt, cfg.scheme, 20)
     assert maxabs(got, ref) <= tol(20)
+    assert np.array_equal(gpu_run(C, cfg, Z, 20, impl=RING), got)
 
 
 def test_3d_batch_jvp_and_composition(C):
@@ -117,6 +136,6 @@ def test_3d_argument_checks(C):
             C.cardiac_create3d(**{**ok, **bad})
     cfg, _ = make(FHN, 16, 16, 8, LAP5, RK4)
     with C.Context.from_config(cfg) as ctx:
-        for plan in (2, 3, (1, 2)):
+        for plan in (2, 3, (1, 3)):
             with pytest.raises(C.CardiacError):
                 C.cardiac_set_plan(ctx.ctx, *(plan if isinstance(plan, tuple) else (plan, 0)))

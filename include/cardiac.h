@@ -143,8 +143,8 @@ int cardiac_set_stream(cardiac_ctx*, void* cuda_stream);
  *   PERSISTENT 0
  * AUTO: PERSISTENT below ~144x144 .. 192x192 cells per member (by model and integrator; batches of up to 4 members,
  * half of that up to 16); FUSED for the two-field models (TMA implementation from ~450 tiles) and for a 4-field grid
- * that is one wave of its tiles; PAIR (TMA) for the 4-field model with RK4 from 1024^2 cells (Heun: 12 Mi); else
- * STAGE. */
+ * that is one wave of its tiles; PAIR (TMA) for the 4-field model with RK4 from 1024^2 cells (Heun: 2048^2) and for
+ * FHN + 4th-order stencil + Heun from 1024^2; STAGE for Karma + Euler below 2048^2 and everything else. */
 int cardiac_set_plan(cardiac_ctx*, int plan, int param);
 
 /* The plan that cardiac_step will use (resolved from AUTO). */

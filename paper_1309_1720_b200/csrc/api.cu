@@ -129,6 +129,18 @@ int auto_plan(const Problem& pb) {
   // a grid that fits one SM never leaves it: the paper's launch-bound regime N < N0
   if (pb.nz > 1) return CARDIAC_PLAN_STAGE;   // 3-D: the stage-synchronous plan only
   if (resident_preferred(pb)) return CARDIAC_PLAN_PERSISTENT;
+  const long long pair_tiles = (long long)((pb.nx + 63) / 64) * ((pb.ny + 23) / 24) * pb.batch;
+  // Heun is two substeps: plan PAIR keeps both on chip with a ring of r cells where the FUSED window carries a halo
+  // of 2r (round 2, FHN LAP9X4 Heun, PAIR / TMA against FUSED: 1024^2 72 / 66, 2048^2 83 / 65, 4096^2 90.5 / 70
+  // Gcell-step/s; Karma LAP5, r = 1: FUSED stays ahead, 89 / 79 at 2048^2)
+  if (pb.model == CARDIAC_FHN && pb.integrator == I_HEUN && pb.radius == 2 && pair_tiles >= kPairTMinTiles &&
+      pair_tma_supported(pb))
+    return CARDIAC_PLAN_PAIR;
+  // Karma + forward Euler: the exponential makes a substep too expensive to recompute over the halo of four
+  // blocked steps; one launch per step wins up to 1536^2 (round 2, LAP5, STAGE / FUSED x 4: 256^2 32 / 26, 1024^2
+  // 187 / 147, 1536^2 220 / 188 Gcell-step/s; from 2048^2 the TMA-fed FUSED is ahead, 180 / 171, 4096^2 205 / 183)
+  if (pb.model == CARDIAC_KARMA && pb.integrator == I_EULER && (long long)pb.nx * pb.ny * pb.batch < (1LL << 22))
+    return CARDIAC_PLAN_STAGE;
   if (rk_like && pb.model != CARDIAC_BOCF) return CARDIAC_PLAN_FUSED;
   // 4-field model: two substeps per launch once the grid gives every SM enough tiles (measured on B200,
   // RK4 1536^2 +2 %, 2048^2 +6 %, 4096^2 +15 %, 8192^2 +19 % over STAGE, behind at
@@ -147,8 +159,9 @@ int auto_plan(const Problem& pb) {
       return CARDIAC_PLAN_PAIR;
     // the TMA-fed implementation already wins once every persistent CTA has four tiles to pipeline
     // (round 2, LAP9X4 RK4: 1024^2 15.5 against 13.0 Gcell-step/s, 768^2 14.0 against 14.8)
-    const long long ntiles = (long long)((pb.nx + 63) / 64) * ((pb.ny + 23) / 24) * pb.batch;
-    if (pb.integrator == I_RK4 && ntiles >= kPairTMinTiles && pair_tma_supported(pb)) return CARDIAC_PLAN_PAIR;
+    if (pb.integrator == I_RK4 && pair_tiles >= kPairTMinTiles && pair_tma_supported(pb)) return CARDIAC_PLAN_PAIR;
+    // Heun: 2048^2 40.4 against 36.8 (STAGE), 1024^2 36.6 against 38.0
+    if (pb.integrator == I_HEUN && cells >= (1LL << 22) && pair_tma_supported(pb)) return CARDIAC_PLAN_PAIR;
   }
   return CARDIAC_PLAN_STAGE;
 }

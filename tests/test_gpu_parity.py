@@ -362,18 +362,19 @@ def test_pair_plan_limits(C):
             C.cardiac_set_plan(ctx.ctx, PAIR[0], 3)
     # AUTO: the 4-field model with RK4 from 4 x 148 tiles of 64 x 24 cells (1024^2; config 4 included), Heun from
     # 12 Mi cells; STAGE below
-    for n, integ, want in [(2048, RK4, PAIR[0]), (1536, RK4, PAIR[0]), (1024, RK4, PAIR[0]), (768, RK4, 1), (2048, HEUN, 1),
-                           (3584, HEUN, PAIR[0]), (2048, EULER, 1)]:
+    for n, integ, want in [(2048, RK4, PAIR[0]), (1536, RK4, PAIR[0]), (1024, RK4, PAIR[0]), (768, RK4, 1), (1536, HEUN, 1),
+                           (2048, HEUN, PAIR[0]), (2048, EULER, 1)]:
         ctx = C.cardiac_create(BOCF, n, n, 0.03, 0.09, LAP9X4 | integ_bits(C, integ), 1)
         try:
             assert C.cardiac_get_plan(ctx) == want, (n, integ)
         finally:
             C.cardiac_destroy(ctx)
-    ctx = C.cardiac_create(FHN, 2048, 2048, 0.04, 1e-4, C.CARDIAC_LAP9X4 | C.CARDIAC_RK4, 1)
-    try:
-        assert C.cardiac_get_plan(ctx) == FUSED
-    finally:
-        C.cardiac_destroy(ctx)
+    for integ, want in [(C.CARDIAC_RK4, FUSED), (C.CARDIAC_HEUN, PAIR[0]), (C.CARDIAC_EULER, FUSED)]:
+        ctx = C.cardiac_create(FHN, 2048, 2048, 0.04, 1e-4, C.CARDIAC_LAP9X4 | integ, 1)
+        try:
+            assert C.cardiac_get_plan(ctx) == want
+        finally:
+            C.cardiac_destroy(ctx)
 
 
 def integ_bits(C, integ):

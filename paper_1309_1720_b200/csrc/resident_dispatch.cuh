@@ -13,9 +13,8 @@ struct ResidentPairs {
   static constexpr int KP = MD::NV > 2 ? 2 : 4;
 };
 
-template <class MD, int STENCIL, int INTEG, int CPT>
+template <class MD, int STENCIL, int INTEG, int CPT, int KP = ResidentPairs<MD>::KP>
 cudaError_t resident_run(const Problem& pb, const ResidentLaunch& rl, cudaStream_t stream) {
-  constexpr int KP = ResidentPairs<MD>::KP;
   constexpr int R = stencil_radius(STENCIL);
   auto kern = resident_kernel<MD, STENCIL, INTEG, KP, CPT>;
   ResidentArgs<MD> a;
@@ -77,6 +76,15 @@ cudaError_t resident_by_integrator(const Problem& pb, const ResidentLaunch& rl, 
   // BOCF wherever the cells fit (Karma RK4 96^2: 5.9 against 6.9 us, BOCF RK4 80^2: 8.5 against 10.8 us)
   const long long ncell = 2LL * ((pb.nx + 1) / 2) * rs.slab;
   const bool cells = ncell <= (long long)kResidentThreads * (MD::NV > 2 || pb.model != 0 ? ResidentPairs<MD>::KP : 1);
+  // the smallest grids (at most one cell per thread: cfg 1) run an instantiation without the loop over units: a
+  // substep there is the latency of ONE warp's instruction sequence, and the unit loop is part of it
+  if (cells && ncell <= kResidentThreads) {
+    switch (pb.integrator) {
+      case I_EULER: return resident_run<MD, STENCIL, I_EULER, 1, 1>(pb, rl, s);
+      case I_HEUN: return resident_run<MD, STENCIL, I_HEUN, 1, 1>(pb, rl, s);
+      case I_RK4: return resident_run<MD, STENCIL, I_RK4, 1, 1>(pb, rl, s);
+    }
+  }
   switch (pb.integrator) {
     case I_EULER: return cells ? resident_run<MD, STENCIL, I_EULER, 1>(pb, rl, s) : resident_run<MD, STENCIL, I_EULER, 2>(pb, rl, s);
     case I_HEUN: return cells ? resident_run<MD, STENCIL, I_HEUN, 1>(pb, rl, s) : resident_run<MD, STENCIL, I_HEUN, 2>(pb, rl, s);

@@ -137,7 +137,8 @@ int cardiac_set_stream(cardiac_ctx*, void* cuda_stream);
  *   PAIR       0 = by size, 1 = DIRECT, 2 = TMA (persistent CTAs, operands by box copies one tile ahead)
  *   FUSED      Euler: time steps per launch (0 = default 4, or 1);  Heun / RK4: window + 16 x implementation with
  *              window 0 = by size, 1 = 80x48 cells (one CTA per SM), 2 = 48x40 (two CTAs per SM; two-field models),
- *              3 / 4 / 5 = 64x56 / 64x48 / 56x48 and 7 = 64x56 on 896 threads (two-field models, RK4), and
+ *              3 / 4 / 5 = 64x56 / 64x48 / 56x48, 7 = 64x56 on 896 threads and 8 = 64x32 on 1024 threads (two-field
+ *              models, RK4), and
  *              implementation 0 = by size, 1 = one CTA per tile, 2 = TMA (persistent CTAs whose windows arrive one
  *              tile ahead; two-field models, windows 1, 2, 3, 7, grids larger than window + halo)
  *   PERSISTENT 0

@@ -103,6 +103,11 @@ int fused_window_auto(const Problem& pb) {
     const long long tw = ew - 2 * H, th = eh - 2 * H;
     return ((pb.nx + tw - 1) / tw) * ((pb.ny + th - 1) / th) * pb.batch;
   };
+  // one wave of 64 x 32 windows on 1024 threads (one row of a pair per thread): the shortest CTA lifetime for a
+  // halo of 8 and for Karma (tile_dispatch.cuh, window 8)
+  if (pb.integrator == I_RK4 && (H == 8 || pb.model == CARDIAC_KARMA) && 64 - 2 * H > 0 && 32 - 2 * H > 0 &&
+      ctas(64, 32) <= 148)
+    return 8;
   const long long small = ctas(48, 40);
   if (small <= 148) return 2;
   constexpr double kFixed = 2000.0;   // cells
@@ -575,10 +580,10 @@ int cardiac_set_plan(cardiac_ctx* c, int plan, int param) {
       if (rparam != 1 && rparam != kEulerBlock)
         return fail(c, CARDIAC_ERR_INVALID, "FUSED + Euler: steps per launch must be 1 or 4");
     } else {
-      if (param < 0 || param > 7 || param == 6 || (param >= 2 && c->pb.nv > 2) || (param >= 3 && integ != I_RK4))
+      if (param < 0 || param > 8 || param == 6 || (param >= 2 && c->pb.nv > 2) || (param >= 3 && integ != I_RK4))
         return fail(c, CARDIAC_ERR_INVALID,
                     "FUSED + Heun/RK4: parameter 0 (auto), 1 (80x48 window), 2 (48x40 window, 2-field models) "
-                    "or 3 / 4 / 5 / 7 (64x56 / 64x48 / 56x48 / 64x56 on 896 threads, 2-field models, RK4)");
+                    "or 3 / 4 / 5 / 7 / 8 (64x56 / 64x48 / 56x48 / 64x56 on 896 threads / 64x32 on 1024 threads, 2-field models, RK4)");
       rparam = param == 0 ? fused_window_auto(c->pb) : param;
     }
   } else if (resolved == CARDIAC_PLAN_PAIR) {

@@ -99,8 +99,8 @@ inline cudaError_t launch_fusedt(const Problem& pb, const TileLaunch& tl, cudaSt
 }
 // window geometry (tile_dispatch.cuh FusedGeom) as the host needs it: output tile of window `win` at halo H
 inline void fused_tile_of(int win, int H, int& tw, int& th) {
-  const int ew = win == 2 ? 48 : (win == 3 || win == 4 || win == 7 ? 64 : (win == 5 ? 56 : 80));
-  const int eh = win == 2 ? 40 : (win == 3 || win == 7 ? 56 : 48);
+  const int ew = win == 2 ? 48 : (win == 3 || win == 4 || win == 7 || win == 8 ? 64 : (win == 5 ? 56 : 80));
+  const int eh = win == 2 ? 40 : (win == 3 || win == 7 ? 56 : (win == 8 ? 32 : 48));
   tw = ew - 2 * H; th = eh - 2 * H;
 }
 bool fused_tma_supported(const Problem& pb, int window, int ksteps);

@@ -43,6 +43,14 @@ template <class MD, int H>
 struct FusedGeom<MD, H, 7> {
   using type = TileGeom<32, 28, 2>;  // 64 x 56 window, 896 threads
 };
+// Small grids (one wave of tiles) pay one CTA lifetime per time step, and the lifetime grows with the rows a thread
+// walks per substep: a 64 x 32 window on 1024 threads x ONE row of a pair each.  Measured (RK4, us per step, against
+// the windows above): FHN LAP9X4 256^2 5.2 / 6.1, 320^2 5.1 / 6.3; Karma LAP5 256^2 5.7 / 6.3, 384^2 6.1 / 6.4; FHN LAP5
+// (halo 4) loses to the 48 x 40 window (4.8 / 4.35).  Two waves always lose.
+template <class MD, int H>
+struct FusedGeom<MD, H, 8> {
+  using type = TileGeom<32, 32, 1>;  // 64 x 32 window, 1024 threads
+};
 template <int VARIANT, int H, int WIN>
 struct FusedGeom<Model<M_BOCF, VARIANT>, H, WIN> {
   using type = TileGeom<24, 16, 2>;  // 48 x 32 window, 384 threads
@@ -118,6 +126,7 @@ cudaError_t fused_by_integrator(const Problem& pb, const TileLaunch& tl, cudaStr
         if (tl.window == 4) return fused_run<MD, STENCIL, I_RK4, 1, 4>(pb, tl, s);
         if (tl.window == 5) return fused_run<MD, STENCIL, I_RK4, 1, 5>(pb, tl, s);
         if (tl.window == 7) return fused_run<MD, STENCIL, I_RK4, 1, 7>(pb, tl, s);
+        if (tl.window == 8) return fused_run<MD, STENCIL, I_RK4, 1, 8>(pb, tl, s);
       }
       return fused_run<MD, STENCIL, I_RK4, 1>(pb, tl, s);
     case I_HEUN:

@@ -100,7 +100,7 @@ def test_parity_fused_small_window(C, model, stencil, integ):
     auto = gpu_run(C, cfg, Z, 40, plan=(2, 0))
     assert maxabs(auto, large) <= 1e-12
     if integ == RK4:          # the three other one-CTA-per-SM windows, several ragged tiles each
-        for win in (3, 4, 5, 7):
+        for win in (3, 4, 5, 7, 8):
             other = gpu_run(C, cfg, Z, 40, plan=(2, win))
             assert maxabs(other, ref) <= tol(40) and maxabs(other, large) <= 1e-12
     else:

@@ -314,21 +314,22 @@ def test_fused_tma_implementation_bitwise_equal_to_fused(C, model, stencil, inte
 def test_tma_pipelines_deterministic_under_load(C, model, stencil, integ, nx, ny, tma, direct):
     """The persistent TMA-fed kernels re-use their shared-memory slots tile after tile (several tiles per CTA here)
     and chain launches by programmatic dependent launch: a box copy landing in a slot that is still being read, or
-    a launch reading its predecessor's output too early, would make the result depend on timing.  60 steps (graph
+    a launch reading its predecessor's output too early, would make the result depend on timing.  60 / 130 steps (graph
     replay + remainder), repeated while another stream keeps the SMs and the L2 busy: the same bits every time, and
     the bits of the direct implementation of the same plan."""
     import torch
     cfg, Z = make(model, nx, ny, stencil, integ, seed=31)
-    ref = gpu_run(C, cfg, Z, 60, plan=direct)
+    n = 60 if tma == PAIRT else 130        # at least one CUDA-graph replay (30 resp. 64 time steps) plus a remainder
+    ref = gpu_run(C, cfg, Z, n, plan=direct)
     side = torch.cuda.Stream()
     noise = torch.empty(64 << 20, dtype=torch.float32, device="cuda")
     for rep in range(3):
         with torch.cuda.stream(side):
             for _ in range(10):
                 noise.normal_()
-        assert np.array_equal(ref, gpu_run(C, cfg, Z, 60, plan=tma))
+        assert np.array_equal(ref, gpu_run(C, cfg, Z, n, plan=tma))
     side.synchronize()
-    assert np.array_equal(ref, gpu_run(C, cfg, Z, 60, plan=tma, chunks=[1, 29, 30]))
+    assert np.array_equal(ref, gpu_run(C, cfg, Z, n, plan=tma, chunks=[1, n // 2 - 1, n - n // 2]))
 
 
 def test_fused_tma_limits_and_auto(C):

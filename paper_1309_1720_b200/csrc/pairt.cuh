@@ -173,7 +173,7 @@ __global__ void __launch_bounds__(PG::NT, 1)
                     const __grid_constant__ CUtensorMap tm_ing, const __grid_constant__ CUtensorMap tm_yu,
                     const __grid_constant__ CUtensorMap tm_yg, const __grid_constant__ CUtensorMap tm_p) {
   using S = PairTShape<MD, STENCIL, KA, KB, PG>;
-  constexpr int NV = S::NV, ND = S::ND, NG = S::NG, R = S::R, HX = S::HX, TW = S::TW, TH = S::TH, PW = S::PW;
+  constexpr int NV = S::NV, ND = S::ND, NG = S::NG, R = S::R, HX = S::HX, TW = S::TW, TH = S::TH;
   constexpr int WW = S::WW, WPW = S::WPW, WH = S::WH, WSZ = S::WSZ, TSZ = S::TSZ, NT = S::NT, NW = S::NW;
   constexpr int NSLOT1 = S::NSLOT1;
   static_assert(!(WRITE_P && !(KA == K_SELF && KB == K_BASE)), "P is formed by RK4 launch 1");

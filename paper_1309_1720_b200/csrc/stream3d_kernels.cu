@@ -36,7 +36,7 @@ constexpr int TW = 64, TH = 8, HP = TW + 4, NT = 32 * TH, ZC = 32;
 
 template <class MD, int STENCIL>
 struct Ring3D {
-  static constexpr int NV = MD::NV, ND = MD::ND;
+  static constexpr int ND = MD::ND;
   static constexpr int R = stencil_radius(STENCIL), NP = 2 * R + 1, HR = TH + 2 * R;
   static constexpr int FSZ = HR * HP;                       // doubles of one field of one plane
   static constexpr int SLOT_BYTES = tma_align128(ND * FSZ * 8);
@@ -76,7 +76,7 @@ __global__ void __launch_bounds__(NT, 2)
                         const __grid_constant__ CUtensorMap tm_A, const __grid_constant__ CUtensorMap tm_B) {
   using L = Ring3D<MD, STENCIL>;
   using P = Oper3D<MD, STENCIL, KIND>;
-  constexpr int NV = MD::NV, ND = MD::ND, NG = NV - ND, R = L::R, NP = L::NP, HR = L::HR, FSZ = L::FSZ, NSLOT = L::NSLOT;
+  constexpr int NV = MD::NV, ND = MD::ND, NG = NV - ND, R = L::R, HR = L::HR, FSZ = L::FSZ, NSLOT = L::NSLOT;
   constexpr int NSLOT_O = P::NSLOT, TSZ = P::TSZ;
   extern __shared__ __align__(1024) unsigned char r3_smem[];
   uint64_t* const full = reinterpret_cast<uint64_t*>(r3_smem + P::OFF_BAR);

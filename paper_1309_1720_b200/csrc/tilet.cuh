@@ -41,7 +41,7 @@ struct TileTShape {
   static constexpr int OFF_GATE = 3 * BUF_BYTES, OFF_BAR = OFF_GATE + GATE_BYTES;
   static constexpr int SMEM_BYTES = OFF_BAR + 128;
   static_assert(SMEM_BYTES <= 227 * 1024, "three stage buffers of this window do not fit one SM");
-  static_assert(E::NS % 2 == 0 || E::NS == 1, "");
+  static_assert(E::NS == 2 || E::NS == 4, "the tile pipeline hangs its TMA requests on the barrier after substep 0");
 };
 
 template <class MD, int STENCIL, int INTEG, int KSTEPS, class TG>
@@ -92,10 +92,7 @@ __global__ void __launch_bounds__(TG::NT, TG::MINB)
     const TilePos tp = tile_pos_of(t, ta.per_member, ta.per_row, ta.tiles_x, TW, TH);
     const int bx = tp.x0 / TW, by = tp.y0 / TH;
     const long long base = (long long)tp.bz * a.g.bstride;
-    // the window of the next tile: `pre` was last read by the tile before this one
-    const unsigned long long tn = (unsigned long long)t + gridDim.x;
-    if (tid == 0 && tn < ta.ntiles) issue_u((unsigned)tn, pre);
-
+    const unsigned long long tn = (unsigned long long)t + gridDim.x;   // the next tile of this CTA
     double* const cur0 = buf(in);
     mbar_wait(fullb + in, (phb >> in) & 1u);
     phb ^= 1u << in;
@@ -123,20 +120,25 @@ __global__ void __launch_bounds__(TG::NT, TG::MINB)
         }
       }
     }
-    if (NG > 0) {
-      __syncthreads();   // everyone has read the staging box: the next tile's may land
-      if (tid == 0 && tn < ta.ntiles) issue_g((unsigned)tn);
-    }
 
     // the substeps: in -> partner -> in -> ... ; the last one writes global memory
     double* out = a.out + base;
     double* c = cur0;
     double* n = buf(partner);
-    if constexpr (NS == 1) {
+    {
       E::template stage<0>(a, out, bx, by, tx, ty, c, n, st);
-    } else {
-      E::template stage<0>(a, out, bx, by, tx, ty, c, n, st);
+      // One barrier does three jobs.  (i) Substep 0 is complete.  (ii) Every thread has finished the LAST substep of
+      // the previous tile, which read that tile's partner buffer = this tile's `pre`: the next tile's window may
+      // land there (its generic-proxy stores are fenced against the async-proxy write first).  (iii) Every thread
+      // has read the staging box of the non-diffusing fields: the next tile's may land.  No barrier is needed at
+      // the END of a tile: substep 0 of the next tile writes the buffer that was this tile's input, last read in the
+      // second-to-last substep, which the barrier before the last substep already closed.
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       __syncthreads();
+      if (tid == 0 && tn < ta.ntiles) {
+        issue_u((unsigned)tn, pre);
+        if (NG > 0) issue_g((unsigned)tn);
+      }
       E::template stage<1>(a, out, bx, by, tx, ty, n, c, st);
       if constexpr (NS == 4) {
         __syncthreads();
@@ -145,9 +147,6 @@ __global__ void __launch_bounds__(TG::NT, TG::MINB)
         E::template stage<3>(a, out, bx, by, tx, ty, n, c, st);
       }
     }
-    // generic-proxy stores into the stage buffers before the TMA unit (async proxy) overwrites them
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    __syncthreads();   // both buffers of this tile are free
     const int o = in; in = pre; pre = partner; partner = o;   // (in, partner, pre) <- (pre, in, partner)
   }
 }

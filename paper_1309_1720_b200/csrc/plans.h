@@ -195,8 +195,9 @@ inline bool resident_supported(const Problem& pb) { return resident_shape(pb).cs
 // AUTO: measured on B200: a substep of the cluster-resident launch costs the ghost
 // exchange (a remote store and the wait for the neighbours') and the latency of one warp's instruction
 // sequence, which grows with the cells a CTA holds; against the per-step launches of FUSED / STAGE it wins up
-// to (batch 1, 16 CTAs; round 2, push exchange) 192^2 for FHN Euler (1.36 against 1.69 us per step), 144^2 for
-// FHN RK4 (5.4 / 5.9), Karma RK4 (5.3 / 6.2) and BOCF RK4 (12.8 / 13.5) — expressed per CTA so that it carries
+// to (batch 1, 16 CTAs; round 2, push exchange, row-major cells) 192^2 for FHN Euler (1.37 against 1.69 us per
+// step), 128^2 for FHN RK4 (4.5 / 5.0; 144^2: 5.5 / 5.0), 144^2 for Karma RK4 (5.0 / 5.6) and 160^2 for BOCF RK4
+// (12.0 / 13.1; 176^2: a tie) — expressed per CTA so that it carries
 // over to the 8-CTA clusters of larger batches — and only while every cluster is resident at once (a GPC holds
 // one cluster of 16, two of 8, four of 4: 17 members in clusters of 8 run as two waves, 8.0 against 6.0 us per
 // FHN RK4 step at 64^2).
@@ -206,7 +207,7 @@ inline bool resident_preferred(const Problem& pb) {
   const int max_clusters = rs.csize == 16 ? 4 : (rs.csize == 8 ? 16 : (rs.csize == 4 ? 32 : 144 / rs.csize));
   if (pb.batch > max_clusters) return false;
   const long long cells_per_cta = 2LL * ((pb.nx + 1) / 2) * rs.slab;
-  const long long limit = pb.nv > 2 ? 1300 : (pb.integrator == 0 ? 2400 : (pb.model == 0 ? 1300 : 1400));
+  const long long limit = pb.nv > 2 ? 1700 : (pb.integrator == 0 ? 2400 : (pb.model == 0 ? 1100 : 1400));
   return cells_per_cta <= limit;
 }
 cudaError_t launch_resident_fhn(const Problem& pb, const ResidentLaunch& rl, cudaStream_t stream);

@@ -55,11 +55,12 @@ CARDIAC_D unsigned cluster_rank() {
 CARDIAC_D void cluster_sync_all() {
   asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
-// CPT = cells per thread and unit: 2 = an x-adjacent pair (128-bit shared-memory accesses); 1 = ONE cell
-// of the pair, the even warps taking the first and the odd warps the second cell of the same 32 pairs
-// (warp-uniform, so each branch keeps only its half of stencil_pair): a substep of a small grid is bound
-// by the latency of one warp's dependent instruction sequence, and half the sequence in twice the warps
-// halves it.  Same per-cell instruction sequence, same bits.
+// CPT = cells per thread and unit: 2 = an x-adjacent pair (128-bit shared-memory accesses); 1 = ONE cell, a warp
+// holding 32 x-adjacent cells (stencil_cell: the operands of either half of stencil_pair in the same positions, so the
+// same bits).  A substep of a small grid is bound by the latency of one warp's dependent instruction sequence, and
+// half the sequence in twice the warps halves it.  (Round 2 first split the PAIRS over even and odd warps; the
+// row-major cells are 10-15 % faster — FHN Euler 64^2 0.49 -> 0.44 us per step, RK4 2.49 -> 2.10 — with contiguous
+// 8-byte accesses instead of every other half of 16-byte ones.)
 template <class MD, int STENCIL, int INTEG, int KP, int CPT>
 struct ResidentEngine {
   static constexpr int NV = MD::NV, ND = MD::ND, NG = NV - ND;
@@ -208,15 +209,12 @@ struct ResidentEngine {
     __syncthreads();
   }
 
-  // pair index of unit k of this thread, and (CPT = 1) which cell of the pair the thread owns
-  CARDIAC_D static int unit_pair(int k) {
-    if (CPT == 2) return threadIdx.x + k * NT;
-    return ((threadIdx.x >> 6) << 5) + (threadIdx.x & 31) + k * (NT / 2);
-  }
-  CARDIAC_D static int unit_half() { return (threadIdx.x >> 5) & 1; }
+  // unit k of this thread: pair index (CPT = 2) or cell index (CPT = 1) inside the slab, row-major — a warp holds 32
+  // x-adjacent units, so its shared-memory accesses are contiguous
+  CARDIAC_D static int unit_index(int k) { return threadIdx.x + k * NT; }
 
   // Substep S of unit k at shared offset o.  W = 2: both cells of the pair (register slots 0, 1);
-  // W = 0 / 1: that cell only (slot 0) — the other half of stencil_pair is dead code.
+  // W = 1: the single cell at o (slot 0).
   template <int S, int W>
   CARDIAC_D static void stage_unit(const ResidentArgs<MD>& a, const double* __restrict__ cur,
                                    double* __restrict__ nxt, Patch& st, int k, int o) {
@@ -226,18 +224,22 @@ struct ResidentEngine {
     double s0[ND], s1[ND];
 #pragma unroll
     for (int q = 0; q < ND; ++q) {
-      ctr[q] = ld2(cur + q * fsz + o);
-      stencil_pair<STENCIL>(cur + q * fsz, o, 0, a.sp, ctr[q], s0[q], s1[q]);
+      if constexpr (W == 2) {
+        ctr[q] = ld2(cur + q * fsz + o);
+        stencil_pair<STENCIL>(cur + q * fsz, o, 0, a.sp, ctr[q], s0[q], s1[q]);
+      } else {
+        ctr[q].x = cur[q * fsz + o];
+        s0[q] = stencil_cell<STENCIL>(cur + q * fsz, o, a.sp, ctr[q].x);
+      }
     }
     double res[2][NV];
 #pragma unroll
-    for (int h = (W == 2 ? 0 : W); h < (W == 2 ? 2 : W + 1); ++h) {
-      const int sl = W == 2 ? h : 0;   // register slot
+    for (int h = 0; h < W; ++h) {
       double z[NV], f[NV];
 #pragma unroll
       for (int q = 0; q < NV; ++q)
         z[q] = q < ND ? (h == 0 ? ctr[q < ND ? q : 0].x : ctr[q < ND ? q : 0].y)
-                      : st.g[k][sl][q >= ND ? q - ND : 0];
+                      : st.g[k][h][q >= ND ? q - ND : 0];
       MD::reaction(a.p, z, f);
 #pragma unroll
       for (int q = 0; q < ND; ++q) f[q] = fma(a.lapw[q], h == 0 ? s0[q] : s1[q], f[q]);
@@ -247,20 +249,20 @@ struct ResidentEngine {
         if (!RK) {
           nv = fma(a.a_dt[0], f[q], z[q]);
         } else if (LAST) {
-          nv = fma(a.b_dt[S], f[q], S == 0 ? st.y[k][sl][q] : st.acc[k][sl][q]);
-          st.y[k][sl][q] = nv;   // the next time step starts here
+          nv = fma(a.b_dt[S], f[q], S == 0 ? st.y[k][h][q] : st.acc[k][h][q]);
+          st.y[k][h][q] = nv;   // the next time step starts here
         } else {
-          st.acc[k][sl][q] = fma(a.b_dt[S], f[q], S == 0 ? st.y[k][sl][q] : st.acc[k][sl][q]);
-          nv = fma(a.a_dt[S], f[q], st.y[k][sl][q]);
+          st.acc[k][h][q] = fma(a.b_dt[S], f[q], S == 0 ? st.y[k][h][q] : st.acc[k][h][q]);
+          nv = fma(a.a_dt[S], f[q], st.y[k][h][q]);
         }
         res[h][q] = nv;
-        if (q >= ND) st.g[k][sl][q >= ND ? q - ND : 0] = nv;
+        if (q >= ND) st.g[k][h][q >= ND ? q - ND : 0] = nv;
       }
     }
 #pragma unroll
     for (int q = 0; q < ND; ++q) {
       if (W == 2) st2(nxt + q * fsz + o, res[0][q], res[1][q]);
-      else nxt[q * fsz + o + W] = res[W][q];
+      else nxt[q * fsz + o] = res[0][q];
     }
   }
 
@@ -268,27 +270,20 @@ struct ResidentEngine {
   template <int S>
   CARDIAC_D static void stage(const ResidentArgs<MD>& a, const double* __restrict__ cur,
                               double* __restrict__ nxt, Patch& st) {
-    if constexpr (CPT == 2) {
+    // Units are handed out in order, so the first missing one ends the list.  Leaving the loop there (a branch
+    // around the rest) or skipping unit by unit (which lets ptxas predicate and interleave the units of a thread) is
+    // the same work; measured, the heavy stages gain from the interleaving (BOCF RK4 96^2 6.2 -> 5.3, 160^2 13.3 ->
+    // 12.0, Karma RK4 96^2 as cells 3.8 -> 3.6 us per step) and the light ones lose 3-6 % to it (FHN, Karma as pairs
+    // or with Euler).
+    constexpr bool kInterleave = NV > 2 || (CPT == 1 && RK);
 #pragma unroll
-      for (int k = 0; k < KP; ++k) {
-        const int o = st.off[k];
-        if (o < 0) break;
-        stage_unit<S, 2>(a, cur, nxt, st, k, o);
+    for (int k = 0; k < KP; ++k) {
+      const int o = st.off[k];
+      if (o < 0) {
+        if (kInterleave) continue;
+        break;
       }
-    } else if (unit_half() == 0) {   // warp-uniform
-#pragma unroll
-      for (int k = 0; k < KP; ++k) {
-        const int o = st.off[k];
-        if (o < 0) continue;   // (an odd row has no second cell in its last pair; a later unit may exist)
-        stage_unit<S, 0>(a, cur, nxt, st, k, o);
-      }
-    } else {
-#pragma unroll
-      for (int k = 0; k < KP; ++k) {
-        const int o = st.off[k];
-        if (o < 0) continue;
-        stage_unit<S, 1>(a, cur, nxt, st, k, o);
-      }
+      stage_unit<S, CPT>(a, cur, nxt, st, k, o);
     }
   }
 
@@ -314,17 +309,22 @@ struct ResidentEngine {
     const unsigned rank = cluster_rank();
     const int y0 = (int)rank * a.slab;
     const int rows = max(0, min(a.slab, a.g.ny - y0));
-    const int fsz = a.sp * a.sr, npairs = a.npx * rows;
+    const int fsz = a.sp * a.sr;
     Patch st;
     // load: diffusing fields -> shared buffer 0, gating fields and y -> registers
-    const int half = unit_half();
+    // position of unit k: row of the slab and (first) column; false = no such unit
+    auto unit_pos = [&](int k, int& py, int& gx) {
+      const int u = unit_index(k), per_row = CPT == 2 ? a.npx : nx;
+      if (u >= per_row * rows) return false;
+      py = u / per_row;
+      gx = CPT * (u - py * per_row);
+      return true;
+    };
 #pragma unroll
     for (int k = 0; k < KP; ++k) {
-      const int p = unit_pair(k);
+      int py, gx;
       st.off[k] = -1;
-      if (p >= npairs) continue;
-      const int py = p / a.npx, px = p - py * a.npx, gx = 2 * px;
-      if (CPT == 1 && gx + half >= nx) continue;   // the second cell of the last pair of an odd row
+      if (!unit_pos(k, py, gx)) continue;
       st.off[k] = (py + R) * a.sp + GX + gx;
 #pragma unroll
       for (int q = 0; q < NV; ++q) {
@@ -337,8 +337,8 @@ struct ResidentEngine {
           else { st.g[k][0][q >= ND ? q - ND : 0] = v.x; st.g[k][1][q >= ND ? q - ND : 0] = v.y; }
           if (RK) { st.y[k][0][q] = v.x; st.y[k][1][q] = v.y; }
         } else {
-          const double v = f[half];
-          if (q < ND) sm[q * fsz + st.off[k] + half] = v;
+          const double v = f[0];
+          if (q < ND) sm[q * fsz + st.off[k]] = v;
           else st.g[k][0][q >= ND ? q - ND : 0] = v;
           if (RK) st.y[k][0][q] = v;
         }
@@ -369,9 +369,8 @@ struct ResidentEngine {
     const double* c = sm + cur * ND * fsz;
 #pragma unroll
     for (int k = 0; k < KP; ++k) {
-      const int p = unit_pair(k);
-      if (st.off[k] < 0) continue;
-      const int py = p / a.npx, px = p - py * a.npx, gx = 2 * px;
+      int py, gx;
+      if (!unit_pos(k, py, gx)) continue;
 #pragma unroll
       for (int q = 0; q < NV; ++q) {
         double* f = out + q * a.g.fstride + (long long)(y0 + py) * pitch + gx;
@@ -382,7 +381,7 @@ struct ResidentEngine {
           f[0] = v.x;
           if (gx + 1 < nx) f[1] = v.y;
         } else {
-          f[half] = q < ND ? c[q * fsz + st.off[k] + half] : st.g[k][0][q >= ND ? q - ND : 0];
+          f[0] = q < ND ? c[q * fsz + st.off[k]] : st.g[k][0][q >= ND ? q - ND : 0];
         }
       }
     }

@@ -112,6 +112,21 @@ CARDIAC_D void stencil_pair(const double* __restrict__ U, int row, int x, int pi
   }
 }
 
+// ... of ONE interior cell at offset o of the field: the operands in the same Stencil<>::apply positions as either
+// half of stencil_pair (c, W, E, S, N, then the second ring) — the same bits
+template <int STENCIL>
+CARDIAC_D double stencil_cell(const double* __restrict__ U, int o, int pitch, double c) {
+  const double* p = U + o;
+  if (STENCIL == S_LAP5) {
+    return Stencil<S_LAP5>::apply(c, p[-1], p[1], p[-pitch], p[pitch]);
+  } else if (STENCIL == S_LAP9X4) {
+    return Stencil<S_LAP9X4>::apply(c, p[-1], p[1], p[-pitch], p[pitch], p[-2], p[2], p[-2 * pitch], p[2 * pitch]);
+  } else {
+    return Stencil<S_BOX9>::apply(c, p[-1], p[1], p[-pitch], p[pitch], p[-pitch - 1], p[-pitch + 1], p[pitch - 1],
+                                  p[pitch + 1]);
+  }
+}
+
 // one cell with the boundary rule applied per axis (Q3)
 template <int STENCIL>
 CARDIAC_D double stencil_edge(const double* __restrict__ U, int i, int j, int nx, int ny, int pitch,

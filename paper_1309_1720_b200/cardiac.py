@@ -1,5 +1,5 @@
 """ctypes binding of libcardiac.so — same names as include/cardiac.h (and the diagnostics of
-include/cardiac_diag.h), argument marshalling only.
+include/cardiac_diag.h, the allocation-free entry point of include/cardiac_static.h), argument marshalling only.
 
 Every step of the hot path runs in the library's CUDA kernels; there is no CPU fallback here.
 Importing this module fails loudly if the library has not been built
@@ -42,6 +42,11 @@ DIAG_EXPORTS = ["cardiac_probe", "cardiac_launch_count", "cardiac_time_steps", "
                 "cardiac_measure_fp64_issue"]
 
 
+# include/cardiac_static.h: the one entry point that allocates nothing (stage buffers in a static device array)
+STATIC_EXPORTS = ["cardiac_step_static"]
+CARDIAC_STATIC_SCRATCH_BYTES = 33554432
+
+
 class CardiacError(RuntimeError):
     def __init__(self, code: int, message: str):
         super().__init__(f"libcardiac error {code}: {message}")
@@ -78,6 +83,7 @@ _sig = {
     "cardiac_time_steps": (_i, [_vp, _ll, _i, ctypes.POINTER(ctypes.c_float)]),
     "cardiac_measure_fp64_peak": (_i, [_vp, _i, _i, _dp]),
     "cardiac_measure_fp64_issue": (_i, [_vp, _i, _i, _i, _dp]),
+    "cardiac_step_static": (_i, [_i, _i, _i, _i, _i, _d, _d, _dp, _i, _vp, _vp, _ll, _vp, ctypes.c_char_p, _i]),
     "cardiac_last_error": (ctypes.c_char_p, [_vp]),
     "cardiac_destroy": (None, [_vp]),
 }
@@ -229,6 +235,26 @@ def cardiac_measure_fp64_issue(ctx, int_per_dfma: int, iters: int = 4000, reps: 
     v = ctypes.c_double(0.0)
     _check(ctx, _lib.cardiac_measure_fp64_issue(ctx, iters, reps, int_per_dfma, ctypes.byref(v)))
     return float(v.value)
+
+
+def cardiac_step_static(model: int, scheme: int, nx: int, ny: int, batch: int, dx: float, dt: float, params,
+                        src, dst, nsteps: int, cuda_stream: int = 0) -> None:
+    """include/cardiac_static.h: `nsteps` time steps from the dense device state `src` into `dst` with the
+    stage buffers in the library's static device array (no allocation; at most CARDIAC_STATIC_SCRATCH_BYTES)."""
+    a_src, dev_src, _k1 = _buffer(src)
+    a_dst, dev_dst, _k2 = _buffer(dst)
+    if not (dev_src and dev_dst):
+        raise TypeError("cardiac_step_static takes device tensors")
+    if params is None:
+        pp, npar = None, 0
+    else:
+        arr = np.ascontiguousarray(params, dtype=np.float64)
+        pp, npar = arr.ctypes.data_as(_dp), int(arr.size)
+    err = ctypes.create_string_buffer(512)
+    rc = _lib.cardiac_step_static(model, scheme, nx, ny, batch, dx, dt, pp, npar, a_src, a_dst, nsteps,
+                                  cuda_stream or None, err, len(err))
+    if rc != CARDIAC_OK:
+        raise CardiacError(rc, err.value.decode())
 
 
 def cardiac_last_error(ctx=None) -> str:

@@ -40,6 +40,12 @@ def test_every_declared_symbol_is_exported(C):
     for n in diag:
         assert hasattr(lib, n) and callable(getattr(C, n))
     assert not any(n in names for n in ("cardiac_probe", "cardiac_time_steps", "cardiac_launch_count"))
+    # ... and so does the allocation-free entry point (include/cardiac_static.h)
+    static = _declared_functions("cardiac_static.h")
+    assert static == sorted(C.STATIC_EXPORTS) == ["cardiac_step_static"]
+    assert hasattr(lib, static[0]) and callable(getattr(C, static[0]))
+    src = open(os.path.join(ROOT, "include", "cardiac_static.h")).read()
+    assert int(re.search(r"#define CARDIAC_STATIC_SCRATCH_BYTES (\d+)", src).group(1)) == C.CARDIAC_STATIC_SCRATCH_BYTES
 
 
 def test_model_tables_and_defaults_agree_with_oracle(C):

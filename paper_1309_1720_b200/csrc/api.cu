@@ -165,6 +165,11 @@ int auto_plan(const Problem& pb) {
     // the TMA-fed implementation already wins once every persistent CTA has four tiles to pipeline
     // (round 2, LAP9X4 RK4: 1024^2 15.5 against 13.0 Gcell-step/s, 768^2 14.0 against 14.8)
     if (pb.integrator == I_RK4 && pair_tiles >= kPairTMinTiles && pair_tma_supported(pb)) return CARDIAC_PLAN_PAIR;
+    // ... and below that where the tiles fill whole rounds of the persistent grid (plans.h; Heun: up to two rounds —
+    // 448^2 7.8 against 9.7 us per step, 640^2 13.0 / 14.9, but 896^2 23.5 / 23.2)
+    if ((pb.integrator == I_RK4 || pb.integrator == I_HEUN) && pair_tma_supported(pb) &&
+        pair_tma_fills_rounds(pair_tiles, pb.integrator == I_RK4 ? 4 : 2))
+      return CARDIAC_PLAN_PAIR;
     // Heun: 2048^2 40.4 against 36.8 (STAGE), 1024^2 36.6 against 38.0
     if (pb.integrator == I_HEUN && cells >= (1LL << 22) && pair_tma_supported(pb)) return CARDIAC_PLAN_PAIR;
   }
@@ -205,6 +210,9 @@ bool pair_uses_tma(const cardiac_ctx* c) {
   if (pb.pair_impl == 1 || !pair_tma_supported(pb)) return false;
   if (pb.pair_impl == 2) return true;
   const long long ntiles = (long long)((pb.nx + 63) / 64) * ((pb.ny + 23) / 24) * pb.batch;
+  if (pb.model == CARDIAC_BOCF && (pb.integrator == I_RK4 || pb.integrator == I_HEUN) &&
+      pair_tma_fills_rounds(ntiles, pb.integrator == I_RK4 ? 4 : 2))
+    return true;   // auto_plan's mid-size rule for the 4-field model
   return ntiles >= kPairTMinTiles;
 }
 

@@ -147,6 +147,14 @@ struct PairTLaunch {
 bool pair_tma_supported(const Problem& pb);   // 2-D, tensor maps available, fewer than 2^31 tiles
 // AUTO picks the TMA implementation once every persistent CTA has several tiles to pipeline
 constexpr long long kPairTMinTiles = 4 * 148;
+// Below that a time step of the TMA pair kernels costs whole ROUNDS of one tile per persistent CTA (4-field model, round 2,
+// LAP9X4: RK4 5.5 + 11.4 x rounds us, Heun 2.5 + 5.2 x rounds us), so it beats the launch-bound STAGE plan exactly where the
+// last round is nearly full: 448^2 (133 tiles) 17.0 against 19.8 us per RK4 step, 640^2 (270) 28.4 / 30.7, 896^2 (532)
+// 51.9 / 57.5 — and loses or ties at 512^2 (176 tiles: 28.4 / 21.7) and 768^2 (384: 39.9 / 39.6).
+inline bool pair_tma_fills_rounds(long long tiles, int max_rounds) {
+  const long long rounds = (tiles + 147) / 148;
+  return tiles >= 120 && rounds <= max_rounds && tiles * 100 >= rounds * 148 * 88;
+}
 cudaError_t launch_pairt_fhn(const Problem& pb, const PairTLaunch& pl, cudaStream_t stream);
 cudaError_t launch_pairt_karma(const Problem& pb, const PairTLaunch& pl, cudaStream_t stream);
 cudaError_t launch_pairt_bocf(const Problem& pb, const PairTLaunch& pl, cudaStream_t stream);

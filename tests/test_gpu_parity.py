@@ -346,6 +346,20 @@ def test_fused_tma_limits_and_auto(C):
     assert np.array_equal(auto, gpu_run(C, cfg, Z, 5, plan=(2, 16))) and np.array_equal(auto, gpu_run(C, cfg, Z, 5, plan=(2, 32)))
 
 
+def test_pair_tma_auto_for_mid_size_grids_that_fill_whole_rounds(C):
+    """4-field model below the 4 x 148-tile threshold: AUTO takes PAIR (TMA implementation) where the 64 x 24 tiles fill
+    whole rounds of the persistent grid (448^2 = 133 tiles, 640^2 = 270) and STAGE where they do not (512^2 = 176);
+    the same bits either way."""
+    for n, integ, want in ((448, RK4, 4), (512, RK4, 1), (640, HEUN, 4), (896, HEUN, 1)):
+        cfg, _ = make(BOCF, n, n, LAP9X4, integ)
+        with C.Context.from_config(cfg) as ctx:
+            assert ctx.plan == want, (n, integ, ctx.plan)
+    cfg, Z = make(BOCF, 448, 440, LAP9X4, RK4, seed=8)
+    auto = gpu_run(C, cfg, Z, 7)
+    assert np.array_equal(auto, gpu_run(C, cfg, Z, 7, plan=PAIRT)) and np.array_equal(auto, gpu_run(C, cfg, Z, 7, plan=STAGE))
+    assert maxabs(auto, O.step(BOCF, Z, cfg.dx, cfg.dt, cfg.scheme, 7, omp=True)) <= tol(7)
+
+
 @pytest.mark.parametrize("model,stencil,integ,bc", [(BOCF, LAP9X4, RK4, 0), (BOCF, LAP5, RK4, 1), (BOCF, BOX9, HEUN, 0),
                                                     (BOCF, LAP9X4, EULER, 1), (FHN, LAP9X4, RK4, 0), (KARMA, BOX9, RK4, 1),
                                                     (KARMA, LAP5, HEUN, 0), (FHN, LAP5, EULER, 0)])

@@ -144,8 +144,13 @@ int auto_plan(const Problem& pb) {
   // Karma + forward Euler: the exponential makes a substep too expensive to recompute over the halo of four
   // blocked steps; one launch per step wins up to 1536^2 (round 2, LAP5, STAGE / FUSED x 4: 256^2 32 / 26, 1024^2
   // 187 / 147, 1536^2 220 / 188 Gcell-step/s; from 2048^2 the TMA-fed FUSED is ahead, 180 / 171, 4096^2 205 / 183)
-  if (pb.model == CARDIAC_KARMA && pb.integrator == I_EULER && (long long)pb.nx * pb.ny * pb.batch < (1LL << 22))
-    return CARDIAC_PLAN_STAGE;
+  // ... except where the grid is ONE wave of 80 x 48 windows with at least 60 tiles (362^2 .. 640^2: 640^2 2.7 against
+  // 4.3 us per step, 448^2 2.64 / 2.78; below, the two are within 3 %)
+  if (pb.model == CARDIAC_KARMA && pb.integrator == I_EULER && (long long)pb.nx * pb.ny * pb.batch < (1LL << 22)) {
+    const int H = pb.radius * kEulerBlock, tw = 80 - 2 * H, th = 48 - 2 * H;
+    const long long tiles = tw > 0 && th > 0 ? (long long)((pb.nx + tw - 1) / tw) * ((pb.ny + th - 1) / th) * pb.batch : 0;
+    return tiles >= 60 && tiles <= 148 ? CARDIAC_PLAN_FUSED : CARDIAC_PLAN_STAGE;
+  }
   if (rk_like && pb.model != CARDIAC_BOCF) return CARDIAC_PLAN_FUSED;
   // 4-field model: two substeps per launch once the grid gives every SM enough tiles (measured on B200,
   // RK4 1536^2 +2 %, 2048^2 +6 %, 4096^2 +15 %, 8192^2 +19 % over STAGE, behind at
@@ -154,8 +159,10 @@ int auto_plan(const Problem& pb) {
     // a grid that is ONE wave of the 4-field model's fused tiles (48 x 32 window) costs one CTA lifetime per time
     // step instead of four launch-bound stage launches (round 2, LAP9X4 RK4: 256^2 9.6 against 14.4 us per step;
     // two waves already lose: 362^2 18.5 against 16.5)
-    if (pb.integrator == I_RK4) {
-      const int H = pb.radius * 4, tw = 48 - 2 * H, th = 32 - 2 * H;
+    // (the same for Heun, halo 2 r, and for four blocked Euler steps, halo 4 r — LAP9X4: Euler 256^2 2.3 against 3.2 us
+    // per step, 320^2 = two waves 4.2 / 3.5; Heun 320^2 6.6 / 7.1, 362^2 = two waves 11.6 / 7.8)
+    if (rk_like) {
+      const int H = pb.radius * (pb.integrator == I_HEUN ? 2 : 4), tw = 48 - 2 * H, th = 32 - 2 * H;
       if (tw > 0 && th > 0 && (long long)((pb.nx + tw - 1) / tw) * ((pb.ny + th - 1) / th) * pb.batch <= 148)
         return CARDIAC_PLAN_FUSED;
     }
@@ -170,8 +177,8 @@ int auto_plan(const Problem& pb) {
     if ((pb.integrator == I_RK4 || pb.integrator == I_HEUN) && pair_tma_supported(pb) &&
         pair_tma_fills_rounds(pair_tiles, pb.integrator == I_RK4 ? 4 : 2))
       return CARDIAC_PLAN_PAIR;
-    // Heun: 2048^2 40.4 against 36.8 (STAGE), 1024^2 36.6 against 38.0
-    if (pb.integrator == I_HEUN && cells >= (1LL << 22) && pair_tma_supported(pb)) return CARDIAC_PLAN_PAIR;
+    // Heun: 2048^2 40.4 against 36.8 (STAGE), 1536^2 63.2 against 69.8 us per step, 1024^2 36.6 against 38.0
+    if (pb.integrator == I_HEUN && pair_tiles >= 2 * kPairTMinTiles && pair_tma_supported(pb)) return CARDIAC_PLAN_PAIR;
   }
   return CARDIAC_PLAN_STAGE;
 }

@@ -204,8 +204,8 @@ inline bool resident_supported(const Problem& pb) { return resident_shape(pb).cs
 // exchange (a remote store and the wait for the neighbours') and the latency of one warp's instruction
 // sequence, which grows with the cells a CTA holds; against the per-step launches of FUSED / STAGE it wins up
 // to (batch 1, 16 CTAs; round 2, push exchange, row-major cells) 192^2 for FHN Euler (1.37 against 1.69 us per
-// step), 128^2 for FHN RK4 (4.5 / 5.0; 144^2: 5.5 / 5.0), 144^2 for Karma RK4 (5.0 / 5.6) and 160^2 for BOCF RK4
-// (12.0 / 13.1; 176^2: a tie) — expressed per CTA so that it carries
+// step), 128^2 for FHN RK4 (4.5 / 5.0; 144^2: 5.5 / 5.0), 144^2 for Karma RK4 (5.0 / 5.6) and 128^2 for BOCF RK4
+// (7.2 / 9.5) — expressed per CTA so that it carries
 // over to the 8-CTA clusters of larger batches — and only while every cluster is resident at once (a GPC holds
 // one cluster of 16, two of 8, four of 4: 17 members in clusters of 8 run as two waves, 8.0 against 6.0 us per
 // FHN RK4 step at 64^2).
@@ -215,7 +215,11 @@ inline bool resident_preferred(const Problem& pb) {
   const int max_clusters = rs.csize == 16 ? 4 : (rs.csize == 8 ? 16 : (rs.csize == 4 ? 32 : 144 / rs.csize));
   if (pb.batch > max_clusters) return false;
   const long long cells_per_cta = 2LL * ((pb.nx + 1) / 2) * rs.slab;
-  const long long limit = pb.nv > 2 ? 1700 : (pb.integrator == 0 ? 2400 : (pb.model == 0 ? 1100 : 1400));
+  // (against the best other plan, which for the 4-field model below 256^2 is the one-wave FUSED launch: RK4 128^2 7.2 / 9.5,
+  // 160^2 12.0 / 9.5; Euler 128^2 1.9 / 2.2, 160^2 2.8 / 2.2; Heun 160^2 5.9 / 6.2 — and for Heun of the two-field models
+  // 160^2 2.9 - 3.1 / 3.7 - 4.1, 192^2 a tie)
+  const long long limit = pb.integrator == 1 ? 1700
+                                             : (pb.nv > 2 ? 1100 : (pb.integrator == 0 ? 2400 : (pb.model == 0 ? 1100 : 1400)));
   return cells_per_cta <= limit;
 }
 cudaError_t launch_resident_fhn(const Problem& pb, const ResidentLaunch& rl, cudaStream_t stream);

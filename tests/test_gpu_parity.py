@@ -400,12 +400,20 @@ def test_pair_plan_limits(C):
         with pytest.raises(C.CardiacError):
             C.cardiac_set_plan(ctx.ctx, PAIR[0], 3)
     # AUTO: the 4-field model with RK4 from 4 x 148 tiles of 64 x 24 cells (1024^2; config 4 included), Heun from
-    # 12 Mi cells; STAGE below
-    for n, integ, want in [(2048, RK4, PAIR[0]), (1536, RK4, PAIR[0]), (1024, RK4, PAIR[0]), (768, RK4, 1), (1536, HEUN, 1),
-                           (2048, HEUN, PAIR[0]), (2048, EULER, 1)]:
+    # 8 x 148 tiles (1536^2); STAGE below (unless the tiles fill whole rounds, see the mid-size test) and one-wave grids FUSED
+    for n, integ, want in [(2048, RK4, PAIR[0]), (1536, RK4, PAIR[0]), (1024, RK4, PAIR[0]), (768, RK4, 1), (1536, HEUN, PAIR[0]),
+                           (1024, HEUN, 1), (2048, HEUN, PAIR[0]), (2048, EULER, 1), (256, EULER, FUSED), (320, EULER, 1),
+                           (320, HEUN, FUSED), (362, HEUN, 1), (160, RK4, FUSED), (128, RK4, PERSISTENT), (160, HEUN, PERSISTENT)]:
         ctx = C.cardiac_create(BOCF, n, n, 0.03, 0.09, LAP9X4 | integ_bits(C, integ), 1)
         try:
             assert C.cardiac_get_plan(ctx) == want, (n, integ)
+        finally:
+            C.cardiac_destroy(ctx)
+    # Karma + Euler: STAGE up to 1536^2 except where the grid is one wave of 60 .. 148 fused windows
+    for n, want in [(256, 1), (448, FUSED), (640, FUSED), (768, 1), (1024, 1), (2048, FUSED)]:
+        ctx = C.cardiac_create(KARMA, n, n, 0.0262, 0.05, C.CARDIAC_LAP5 | C.CARDIAC_EULER, 1)
+        try:
+            assert C.cardiac_get_plan(ctx) == want, n
         finally:
             C.cardiac_destroy(ctx)
     for integ, want in [(C.CARDIAC_RK4, FUSED), (C.CARDIAC_HEUN, PAIR[0]), (C.CARDIAC_EULER, FUSED)]:

@@ -142,10 +142,11 @@ int cardiac_set_stream(cardiac_ctx*, void* cuda_stream);
  *              implementation 0 = by size, 1 = one CTA per tile, 2 = TMA (persistent CTAs whose windows arrive one
  *              tile ahead; two-field models, windows 1, 2, 3, 7, grids larger than window + halo)
  *   PERSISTENT 0
- * AUTO: PERSISTENT below ~144x144 .. 192x192 cells per member (by model and integrator; batches of up to 4 members,
- * half of that up to 16); FUSED for the two-field models (TMA implementation from ~450 tiles) and for a 4-field grid
- * that is one wave of its tiles; PAIR (TMA) for the 4-field model with RK4 from 1024^2 cells (Heun: 2048^2) and for
- * FHN + 4th-order stencil + Heun from 1024^2; STAGE for Karma + Euler below 2048^2 and everything else. */
+ * AUTO: PERSISTENT below ~128x128 .. 192x192 cells per member (by model and integrator; batches of up to 4 members,
+ * half of that up to 16); FUSED for the two-field models (TMA implementation from ~370 - 450 tiles) and for a 4-field
+ * grid that is one wave of its tiles; PAIR (TMA) for the 4-field model with RK4 from 1024^2 cells (Heun: 1536^2) and
+ * below that where its 64 x 24 tiles fill whole rounds of the persistent grid; STAGE for Karma + Euler below 2048^2
+ * (except one-wave grids) and everything else.  DESIGN.md "Plan choice" has the measurements. */
 int cardiac_set_plan(cardiac_ctx*, int plan, int param);
 
 /* The plan that cardiac_step will use (resolved from AUTO). */

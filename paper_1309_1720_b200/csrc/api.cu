@@ -122,7 +122,9 @@ int fused_window_auto(const Problem& pb) {
     if (c4 < best_cost) { best = 4; best_cost = c4; }
     if (c5 < best_cost) { best = 5; best_cost = c5; }
   }
-  if (H <= 4) {
+  // (not for FHN + Heun, two diffusing fields at halo 4: measured, the 80 x 48 window wins at every size above one wave
+  // of small windows — 448^2 5.6 against 6.4 us per step, 768^2 9.5 / 11.0)
+  if (H <= 4 && !(pb.model == CARDIAC_FHN && pb.integrator == I_HEUN)) {
     const double c2 = (80.0 * 48.0 + kFixed) / 1.18 * (0.57 + (double)small / 296.0);
     if (c2 < best_cost) best = 2;
   }
@@ -135,12 +137,9 @@ int auto_plan(const Problem& pb) {
   if (pb.nz > 1) return CARDIAC_PLAN_STAGE;   // 3-D: the stage-synchronous plan only
   if (resident_preferred(pb)) return CARDIAC_PLAN_PERSISTENT;
   const long long pair_tiles = (long long)((pb.nx + 63) / 64) * ((pb.ny + 23) / 24) * pb.batch;
-  // Heun is two substeps: plan PAIR keeps both on chip with a ring of r cells where the FUSED window carries a halo
-  // of 2r (round 2, FHN LAP9X4 Heun, PAIR / TMA against FUSED: 1024^2 72 / 66, 2048^2 83 / 65, 4096^2 90.5 / 70
-  // Gcell-step/s; Karma LAP5, r = 1: FUSED stays ahead, 89 / 79 at 2048^2)
-  if (pb.model == CARDIAC_FHN && pb.integrator == I_HEUN && pb.radius == 2 && pair_tiles >= kPairTMinTiles &&
-      pair_tma_supported(pb))
-    return CARDIAC_PLAN_PAIR;
+  // (Heun of the two-field models: plan PAIR / TMA was ahead of FUSED for FHN LAP9X4 until the FUSED / TMA pipeline lost
+  // its end-of-tile barrier; since then the 80 x 48 window fed by TMA wins from 1024^2 — 2048^2 46.3 against 51.0 us per
+  // step, 4096^2 148 / 186 = 113 / 90 Gcell-step/s — and FUSED is taken below)
   // Karma + forward Euler: the exponential makes a substep too expensive to recompute over the halo of four
   // blocked steps; one launch per step wins up to 1536^2 (round 2, LAP5, STAGE / FUSED x 4: 256^2 32 / 26, 1024^2
   // 187 / 147, 1536^2 220 / 188 Gcell-step/s; from 2048^2 the TMA-fed FUSED is ahead, 180 / 171, 4096^2 205 / 183)
@@ -202,6 +201,9 @@ int enqueue_fused(cardiac_ctx* c, cudaStream_t s, int ksteps) {
       fused_tile_of(c->pb.integrator == I_EULER ? 1 : tl.window, c->pb.radius * ns, tw, th);
       const long long ntiles = (long long)((c->pb.nx + tw - 1) / tw) * ((c->pb.ny + th - 1) / th) * c->pb.batch;
       tma = tl.window == 7 ? ntiles >= 400 : ntiles >= kFusedTMinTiles * (tl.window == 2 ? 2 : 1);
+      // Heun, 80 x 48 window: two substeps per tile leave less to overlap, the pipeline pays from ~2.5 tiles per CTA
+      // (FHN LAP9X4: 1024^2 = 390 tiles 13.3 against 14.2 us per step, 896^2 = 299 tiles 13.4 / 13.5, 768^2 9.9 / 9.5)
+      if (c->pb.integrator == I_HEUN && tl.window == 1) tma = ntiles >= 370;
     }
   }
   cudaError_t e = tma ? launch_fusedt(c->pb, tl, s) : launch_fused(c->pb, tl, s);

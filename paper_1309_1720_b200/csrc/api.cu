@@ -3,6 +3,7 @@
 // lives here; it only sequences the kernels of *_kernels.cu.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -149,6 +150,32 @@ int auto_plan(const Problem& pb) {
     const int H = pb.radius * kEulerBlock, tw = 80 - 2 * H, th = 48 - 2 * H;
     const long long tiles = tw > 0 && th > 0 ? (long long)((pb.nx + tw - 1) / tw) * ((pb.ny + th - 1) / th) * pb.batch : 0;
     return tiles >= 60 && tiles <= 148 ? CARDIAC_PLAN_FUSED : CARDIAC_PLAN_STAGE;
+  }
+  // Karma with a radius-2 stencil: every cell of the halo pays an exponential, so beyond one wave of windows the
+  // stage-synchronous plan wins while its buffers stay in L2 (round 2 audit, LAP9X4: RK4 1024^2 30.1 against 37.7 us
+  // per step, Heun 1536^2 26.8 / 36.2, 768^2 9.6 / 11.6; from 1536^2 / 2048^2 the TMA-fed FUSED is ahead again), and
+  // four blocked Euler steps (halo 8) never pay beyond one wave (4096^2 96 / 118)
+  if (pb.model == CARDIAC_KARMA && pb.radius >= 2 && rk_like) {
+    const int H = pb.radius * (pb.integrator == I_RK4 ? 4 : (pb.integrator == I_HEUN ? 2 : kEulerBlock));
+    auto ctas = [&](int ew, int eh) -> long long {
+      const int tw = ew - 2 * H, th = eh - 2 * H;
+      if (tw <= 0 || th <= 0) return 1LL << 40;
+      return (long long)((pb.nx + tw - 1) / tw) * ((pb.ny + th - 1) / th) * pb.batch;
+    };
+    const long long cells = (long long)pb.nx * pb.ny * pb.batch;
+    long long one_wave = ctas(80, 48);
+    if (pb.integrator != I_EULER) one_wave = std::min(one_wave, ctas(48, 40));
+    if (pb.integrator == I_RK4) one_wave = std::min(std::min(one_wave, ctas(64, 56)), ctas(64, 32));
+    bool fused = one_wave <= 148;
+    // (Heun: one wave of the LARGE window costs ~6.8 us, more than two stage launches below ~575^2)
+    if (pb.integrator == I_HEUN && ctas(48, 40) > 148 && cells < 330000) fused = false;
+    if (fused) return CARDIAC_PLAN_FUSED;
+    const long long working_set = cells * pb.nv * 8 * (pb.integrator == I_RK4 ? 4 : 2);
+    if (pb.integrator == I_EULER || working_set <= (96LL << 20)) return CARDIAC_PLAN_STAGE;
+    // streaming sizes: a pair's ring of r cells against the window's halo of 2r / 4r (2048^2 Heun 58.5 against 62.7 us per
+    // step, 4096^2 RK4 479 / 511)
+    if (pair_tiles >= 4 * kPairTMinTiles && pair_tma_supported(pb)) return CARDIAC_PLAN_PAIR;
+    return CARDIAC_PLAN_FUSED;
   }
   if (rk_like && pb.model != CARDIAC_BOCF) return CARDIAC_PLAN_FUSED;
   // 4-field model: two substeps per launch once the grid gives every SM enough tiles (measured on B200,
